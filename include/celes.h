@@ -1,0 +1,130 @@
+/* celes.h -- C ABI of the B200-native CELES hot path (arxiv 1706.02145, PAPER.md).
+ *
+ * The library solves the multiple-scattering system of N spheres, eq. (8)-(9) of the paper,
+ *
+ *     sum_{i',n'} M^{ii'}_{nn'} b^{i'}_{n'} = sum_{n'} T^i_{nn'} a^i_{in,n'},   M = 1 - T W,
+ *
+ * with the coupling operator W^{ii'}_{nn'} = A_{n'n}(r_i - r_i') (eq. 7; A from the SVWF
+ * addition theorem (A.5)-(A.11)) evaluated on the fly, never stored, and the
+ * sphere T-matrix diagonal T^i_{nn'} = Q^i_{tau,l} (B.1).
+ *
+ * Conventions
+ *   - Multi-index n = (tau, l, m), tau in {1,2}, l = 1..lmax, m = -l..l; 0-based position
+ *     n = (tau-1) nmax/2 + (l-1)(l+1) + (m+l), nmax = 2 lmax (lmax+2).
+ *   - Coefficient vectors are complex64, interleaved (re, im), laid out [sphere i][n], length N*nmax
+ *     (identical to a contiguous torch.complex64 tensor of shape [N, nmax]).
+ *   - Associated Legendre functions are normalised without Condon-Shortley phase.
+ *   - Lengths are in one unit U (nm in the paper's examples), k in 1/U.
+ *   - Every function returns 0 (CELES_OK) or a negative error code; nothing throws, nothing is printed.
+ *   - "dev" pointers are CUDA device pointers owned by the caller; "host" pointers are plain host memory.
+ *     cuda_stream is a cudaStream_t (NULL = default stream).  The matvec entry points only enqueue work on
+ *     that stream and do not synchronise; celes_solve and the *_host variants synchronise the stream.
+ *   - There is no CPU fallback: without a CUDA device every compute entry point returns CELES_ECUDA.
+ */
+#ifndef CELES_H
+#define CELES_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define CELES_OK       0
+#define CELES_EINVAL  -1   /* bad argument: N < 1, unsupported lmax, null pointer, non-finite input, k <= 0, overlapping spheres */
+#define CELES_ENOMEM  -2   /* host or device allocation failed */
+#define CELES_ECUDA   -3   /* CUDA runtime error (no device, launch failure, ...) */
+#define CELES_ENOCONV -4   /* celes_solve reached max_iters; x holds the last iterate and info is filled */
+
+#define CELES_LMAX_MIN 1
+#define CELES_LMAX_MAX 4
+#define CELES_MAX_HISTORY 4096
+
+typedef struct celes_ctx celes_ctx;   /* opaque; owns every device table; freed by celes_destroy */
+
+/* Options of celes_setup (nullable -> defaults).  Zero in a field selects its default. */
+typedef struct celes_options {
+    int emitter_tile;      /* emitters staged per shared-memory tile; default 32 */
+    int emitter_splits;    /* how many slices the emitter sum of one receiver is cut into (split-K across CTAs);
+                              0 = chosen so that the grid fills a whole number of waves on the device */
+    int skip_overlap_check;/* 1: do not verify that spheres are disjoint */
+} celes_options;
+
+#define CELES_GMRES 0
+typedef struct celes_solve_opts {
+    int method;            /* CELES_GMRES */
+    int restart;           /* GMRES restart length; default 30 */
+    double rtol;           /* stop when ||T a_in - M x||_2 / ||T a_in||_2 <= rtol; default 1e-4 */
+    int max_iters;         /* bound on inner iterations (= system matvecs inside cycles); default 1000 */
+} celes_solve_opts;
+
+typedef struct celes_solve_info {
+    int iterations;        /* inner GMRES iterations performed */
+    int matvecs;           /* system matvecs, including the true-residual evaluations at restarts */
+    int converged;         /* 1 if the TRUE relative residual met rtol */
+    double rel_residual;   /* true relative residual ||T a_in - M x|| / ||T a_in|| of the returned x */
+    double seconds;        /* wall-clock time inside celes_solve */
+    int n_history;         /* entries used in history */
+    double history[CELES_MAX_HISTORY]; /* relative residual estimate after each inner iteration */
+} celes_solve_info;
+
+/* celes_setup -- particle positions, radii, Mie coefficients, k and lmax.
+ *   pos_xyz  host, [N][3] double, sphere centres r_i.
+ *   radii    host, [N] double, R_i; used only to verify that spheres are disjoint (needed for |r| < |d| in A.5).
+ *   mie_q    host, [N][2][lmax] complex128 interleaved: Q^i_{tau,l} of (B.2)-(B.3).
+ *   k        background wavenumber n_0 omega / c > 0.
+ * Builds on the device: k-scaled FP64 centres, the T diagonal, and the a5/b5 translation-coefficient table
+ * (PAPER.md:129, 258-267).  Copies everything it needs; the host arrays may be freed afterwards.
+ * On success *out is a new context; on error *out is NULL. */
+int celes_setup(celes_ctx** out, int N, int lmax, const double* pos_xyz, const double* radii,
+                const double* mie_q, double k, const celes_options* opt, void* cuda_stream);
+
+/* y = W b : y^i_n = sum_{i' != i} sum_{n'} W^{ii'}_{nn'} b^{i'}_{n'}  (eq. 6 without a_in).
+ * b_dev, y_dev: device, N*nmax complex64, must not alias.  Asynchronous on cuda_stream. */
+int celes_coupling_matvec(celes_ctx* ctx, const void* b_dev, void* y_dev, void* cuda_stream);
+
+/* out = M b = b - T (W b)  (eqs. 8-9).  Same argument rules as above. */
+int celes_system_matvec(celes_ctx* ctx, const void* b_dev, void* out_dev, void* cuda_stream);
+
+/* Host-buffer variants: copy b from host memory (pinned or pageable), run the device path, copy the result back,
+ * synchronise.  b_host, y_host: N*nmax complex64. */
+int celes_coupling_matvec_host(celes_ctx* ctx, const void* b_host, void* y_host, void* cuda_stream);
+int celes_system_matvec_host(celes_ctx* ctx, const void* b_host, void* out_host, void* cuda_stream);
+
+/* Solve eq. (8) for the scattered-field coefficients b with a host-driven Krylov loop whose matvecs, dot products,
+ * axpys and norms are device kernels.
+ *   a_in_dev  device, N*nmax complex64: initial-field coefficients a_in (the library forms T a_in).
+ *   x_dev     device, N*nmax complex64: in = initial guess x0 (zero it for x0 = 0), out = b.
+ *   o         nullable -> defaults (GMRES(30), rtol 1e-4, 1000 iterations).
+ *   info      nullable.
+ * Returns CELES_OK, or CELES_ENOCONV with x and info still filled. */
+int celes_solve(celes_ctx* ctx, const void* a_in_dev, void* x_dev, const celes_solve_opts* o,
+                celes_solve_info* info, void* cuda_stream);
+
+/* Release the context and every device table it owns.  NULL is allowed. */
+void celes_destroy(celes_ctx* ctx);
+
+/* Static description of an error code. */
+const char* celes_strerror(int code);
+
+/* Sizes the caller needs: nmax = 2 lmax (lmax+2); returns CELES_EINVAL (<0) for an unsupported lmax. */
+int celes_nmax(int lmax);
+
+/* Grid the coupling kernel of this context is launched with (for reporting): receiver blocks, emitter splits,
+ * threads per block, emitters per tile.  Any pointer may be NULL. */
+int celes_launch_config(const celes_ctx* ctx, int* receiver_blocks, int* emitter_splits, int* block_threads,
+                        int* emitter_tile);
+
+/* Host-only (needs no GPU): the translation coefficients the library uses, for W_{(tau l m),(tau' l' m')}:
+ *   a5_re[((r*H)+c)*P + p] = Re a5(l',m'|l,m|p),  b5_im[...] = Im b5(l',m'|l,m|p)   (eq. 7),
+ * r, c = (l-1)(l+1)+(m+l) of receiver / emitter, H = lmax (lmax+2), P = 2 lmax + 1, p = 0..2 lmax.
+ * Both arrays have H*H*P doubles. */
+int celes_translation_table(int lmax, double* a5_re, double* b5_im);
+
+/* FP32 peak probe: runs an FFMA-only kernel (independent chains, every SM) and reports the achieved
+ * FLOP/s (2 flop per FMA).  variant 0: three-register FFMA; 1: FFMA with an immediate multiplicand;
+ * 2: packed fma.rn.f32x2.  Synchronises the stream. */
+int celes_fp32_peak_probe(int variant, int iters, double* flops_per_s, double* milliseconds, void* cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CELES_H */

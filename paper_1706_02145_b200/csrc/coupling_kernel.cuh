@@ -1,0 +1,164 @@
+// coupling_kernel.cuh -- device kernels of y = W b (steps H1-H9 of DESIGN.md section 5).
+//
+//   pack_kernel      b [N][nmax] -> bpm [N][nmax] = [b_1 + b_2 | b_1 - b_2]      (tau-block symmetry of W)
+//   coupling_kernel  tiled (receiver-block x emitter-block) translation; one thread per receiver, the
+//                    emitter tile (coefficients + FP64 centres) staged through shared memory, FP32 complex
+//                    accumulation in registers (lmax <= 3) or in a conflict-free shared-memory slab (lmax = 4)
+//   finalize_kernel  sums the emitter splits, undoes the +- transform, optional epilogue out = b - T y (eq. 9)
+#pragma once
+#include <cuda_runtime.h>
+
+#include "pair_math.cuh"
+
+namespace celes {
+
+constexpr int kBlock = 128;          // receivers (threads) per CTA
+
+__host__ __device__ constexpr int nmax_of(int lmax) { return 2 * lmax * (lmax + 2); }
+
+// ---------------------------------------------------------------------------------------------------------
+// b -> [b_+ | b_-].  One thread per (sphere, index inside a tau block).
+__global__ void pack_kernel(int N, int H, const float2* __restrict__ b, float2* __restrict__ bpm) {
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= (long long)N * H) return;
+    const long long i = t / H;
+    const int q = (int)(t - i * H);
+    const float2 b1 = b[i * 2 * H + q], b2 = b[i * 2 * H + H + q];
+    bpm[i * 2 * H + q] = make_float2(b1.x + b2.x, b1.y + b2.y);
+    bpm[i * 2 * H + H + q] = make_float2(b1.x - b2.x, b1.y - b2.y);
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// Accumulator policies for y_pm of one receiver.
+template <int NMAX>
+struct YRegs {                       // registers: every index is a literal after unrolling
+    float re[NMAX], im[NMAX];
+    __device__ __forceinline__ void init(float*, int) {
+#pragma unroll
+        for (int q = 0; q < NMAX; ++q) { re[q] = 0.0f; im[q] = 0.0f; }
+    }
+    __device__ __forceinline__ void operator()(int q, float r, float i) { re[q] += r; im[q] += i; }
+    __device__ __forceinline__ float2 get(int q) const { return make_float2(re[q], im[q]); }
+    static constexpr size_t smem_bytes() { return 0; }
+};
+
+template <int NMAX>
+struct YSmem {                       // shared memory slab [q][thread] (float2): lane-contiguous, conflict-free
+    float2* base;
+    __device__ __forceinline__ void init(float* smem, int tid) {
+        base = reinterpret_cast<float2*>(smem) + tid;
+#pragma unroll
+        for (int q = 0; q < NMAX; ++q) base[q * kBlock] = make_float2(0.0f, 0.0f);
+    }
+    __device__ __forceinline__ void operator()(int q, float r, float i) {
+        float2 v = base[q * kBlock];
+        v.x += r; v.y += i;
+        base[q * kBlock] = v;
+    }
+    __device__ __forceinline__ float2 get(int q) const { return base[q * kBlock]; }
+    static constexpr size_t smem_bytes() { return sizeof(float2) * NMAX * kBlock; }
+};
+
+template <int LMAX>
+struct YPolicy { using type = YRegs<nmax_of(LMAX)>; };
+template <>
+struct YPolicy<4> { using type = YSmem<nmax_of(4)>; };
+
+template <int LMAX>
+constexpr size_t coupling_smem_bytes(int etile) {
+    return YPolicy<LMAX>::type::smem_bytes() + (size_t)etile * (nmax_of(LMAX) * sizeof(float2) + 3 * sizeof(double));
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// grid = (ceil(N / kBlock), splits).  CTA (bx, by) translates emitters [by*chunk, min(N, (by+1)*chunk)) to
+// receivers bx*kBlock + tid and writes its partial sums to ypart[by][receiver][q].
+//   kpos  [N][3] FP64: k * r_i.  The subtraction r_i - r_i' is done in FP64, everything after it in FP32.
+template <int LMAX>
+__global__ void __launch_bounds__(kBlock) coupling_kernel(int N, int chunk, int etile,
+                                                          const double* __restrict__ kpos,
+                                                          const float2* __restrict__ bpm,
+                                                          float2* __restrict__ ypart) {
+    constexpr int NMAX = nmax_of(LMAX);
+    using Y = typename YPolicy<LMAX>::type;
+    extern __shared__ __align__(16) float smem_raw[];
+    float* ysm = smem_raw;
+    float2* sb = reinterpret_cast<float2*>(reinterpret_cast<char*>(smem_raw) + Y::smem_bytes());   // [etile][NMAX]
+    double* spos = reinterpret_cast<double*>(sb + (size_t)etile * NMAX);                           // [etile][3]
+
+    const int tid = threadIdx.x;
+    const int i = blockIdx.x * kBlock + tid;
+    const bool active = i < N;
+    const int ic = active ? i : N - 1;
+    const double xi = kpos[3 * ic], yi = kpos[3 * ic + 1], zi = kpos[3 * ic + 2];
+
+    Y yacc;
+    yacc.init(ysm, tid);
+
+    const int e_begin = blockIdx.y * chunk;
+    const int e_end = min(N, e_begin + chunk);
+    for (int t0 = e_begin; t0 < e_end; t0 += etile) {
+        const int ne = min(etile, e_end - t0);
+        __syncthreads();                                       // previous tile fully consumed
+        {   // H1: stage the tile -- coefficients are contiguous in global memory: ne * NMAX float2 = ne*NMAX/2 float4
+            const float4* src = reinterpret_cast<const float4*>(bpm + (size_t)t0 * NMAX);
+            float4* dst = reinterpret_cast<float4*>(sb);
+            const int nvec = ne * NMAX / 2;
+            for (int v = tid; v < nvec; v += kBlock) dst[v] = __ldg(src + v);
+            for (int v = tid; v < 3 * ne; v += kBlock) spos[v] = kpos[(size_t)3 * t0 + v];
+        }
+        __syncthreads();
+        for (int e = 0; e < ne; ++e) {
+            if (t0 + e == i) continue;                         // sum over i' != i (eq. 6)
+            const float dx = (float)(xi - spos[3 * e]);        // d = r_i - r_i' (eq. 7), FP64 subtraction
+            const float dy = (float)(yi - spos[3 * e + 1]);
+            const float dz = (float)(zi - spos[3 * e + 2]);
+            const float2* be = sb + e * NMAX;
+            auto bload = [be](int q) { return be[q]; };        // same address in every lane: LDS broadcast
+            pair_translate<LMAX>(dx, dy, dz, bload, yacc);
+        }
+    }
+    if (active) {
+        float2* dst = ypart + ((size_t)blockIdx.y * N + i) * NMAX;
+#pragma unroll
+        for (int q = 0; q < NMAX; ++q) dst[q] = yacc.get(q);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// H8-H9: y_1 = (y_+ + y_-)/2, y_2 = (y_+ - y_-)/2 summed over the splits; if tdiag != nullptr the epilogue of
+// eq. (9) is fused: out = b - T y with T the diagonal Q^i_{tau,l} expanded to [N][nmax].
+__global__ void finalize_kernel(int N, int H, int splits, const float2* __restrict__ ypart,
+                                const float2* __restrict__ tdiag, const float2* __restrict__ b,
+                                float2* __restrict__ out) {
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= (long long)N * H) return;
+    const long long i = t / H;
+    const int q = (int)(t - i * H);
+    const size_t stride = (size_t)N * 2 * H;
+    float pr = 0.f, pi = 0.f, mr = 0.f, mi = 0.f;
+    for (int s = 0; s < splits; ++s) {
+        const float2 yp = ypart[s * stride + i * 2 * H + q], ym = ypart[s * stride + i * 2 * H + H + q];
+        pr += yp.x; pi += yp.y; mr += ym.x; mi += ym.y;
+    }
+    float2 y1 = make_float2(0.5f * (pr + mr), 0.5f * (pi + mi));
+    float2 y2 = make_float2(0.5f * (pr - mr), 0.5f * (pi - mi));
+    const size_t o1 = i * 2 * H + q, o2 = o1 + H;
+    if (tdiag != nullptr) {
+        const float2 t1 = tdiag[o1], t2 = tdiag[o2], b1 = b[o1], b2 = b[o2];
+        y1 = make_float2(b1.x - (t1.x * y1.x - t1.y * y1.y), b1.y - (t1.x * y1.y + t1.y * y1.x));
+        y2 = make_float2(b2.x - (t2.x * y2.x - t2.y * y2.y), b2.y - (t2.x * y2.y + t2.y * y2.x));
+    }
+    out[o1] = y1;
+    out[o2] = y2;
+}
+
+// out = T a (diagonal), used for the right-hand side of eq. (8)
+__global__ void tapply_kernel(long long n, const float2* __restrict__ tdiag, const float2* __restrict__ a,
+                              float2* __restrict__ out) {
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= n) return;
+    const float2 q = tdiag[t], v = a[t];
+    out[t] = make_float2(q.x * v.x - q.y * v.y, q.x * v.y + q.y * v.x);
+}
+
+}  // namespace celes

@@ -1,0 +1,282 @@
+#!/usr/bin/env python3
+"""bench.py -- coupling-matvec throughput of the CELES hot path on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C4|C3] [--impl ours|reference]
+
+A step is one pass of the whole hot path y = W b (pack -> coupling kernel -> finalize) over the synthetic
+ensemble of BASELINE.json config 4 (N = 1e5 spheres, lmax = 3).  `value` is sphere-pair
+translations per second, N (N-1) / time, inputs resident in HBM; `e2e` is the same metric through
+celes_coupling_matvec_host with pinned HOST buffers (H2D + D2H inside the timed region).
+
+The path does not shard (north_star: one GPU, no collectives): --gpus N runs N independent replicas
+("replicas only"), value = pairs of all replicas / max-over-ranks time.
+
+--impl reference times the FP64 CPU oracle (oracle/), as it stands, on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "sphere_pair_translations_per_s"
+UNIT = "pairs/s"
+# Algorithmic FP32 flops per ordered pair of the direct, tau-symmetric translation (DESIGN.md section 6:
+# counted from the generated pair body, FMA = 2): geometry + radial + angular + p-contraction + n'-contraction.
+FLOPS_PER_PAIR = {3: 8.0e3, 4: 21.8e3}
+FP32_LANES_PER_SM = 128
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="C4")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=20.0, help="CPU work of the cpu_baseline sample")
+    return ap.parse_args()
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (the profiling recipe's clocks line)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.proc, self.path = index, None, None
+
+    def start(self):
+        try:
+            f = tempfile.NamedTemporaryFile("w", suffix=".csv", delete=False)
+            self.path = f.name
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100", "-i", str(self.index)], stdout=f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.proc = None
+
+    def stop(self) -> dict:
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return out
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, reasons, pw = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        try:
+            for line in open(self.path):
+                p = [x.strip() for x in line.split(",")]
+                if len(p) < 9:
+                    continue
+                try:
+                    sm.append(float(p[1])); mx.append(float(p[2])); pw.append(float(p[3]))
+                except ValueError:
+                    continue
+                for nm, v in zip(names, p[5:9]):
+                    if v.lower().startswith("active"):
+                        reasons.add(nm)
+            os.unlink(self.path)
+        except OSError:
+            pass
+        if sm:
+            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), reasons=sorted(reasons),
+                       samples=len(sm), power_w_max=float(max(pw)))
+        return out
+
+
+def measured_peaks() -> dict:
+    try:
+        return json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except (OSError, ValueError):
+        return {}
+
+
+def oracle_sample_rate(w, pos, b, seconds: float):
+    """Times the oracle (as it stands) on whole receivers of workload w until about `seconds` of CPU work."""
+    from oracle import celes_oracle as orc
+    from paper_1706_02145_b200 import workloads
+    t0 = time.perf_counter()
+    orc.coupling_matvec(pos, w.k, w.lmax, b, receivers=np.array([0]))          # calibration: one receiver
+    t1 = time.perf_counter() - t0
+    cores = max(1, orc.LAST_THREADS)
+    per_recv = t1                                                             # one receiver is one thread's work
+    n_recv = int(max(cores, min(w.N, seconds / max(per_recv, 1e-9) * cores)))
+    n_recv = (n_recv // cores) * cores
+    recv = workloads.sample_receivers(w.N, n_recv, 404)
+    t0 = time.perf_counter()
+    orc.coupling_matvec(pos, w.k, w.lmax, b, receivers=recv)
+    dt = time.perf_counter() - t0
+    pairs = len(recv) * (w.N - 1)
+    return pairs / dt, cores, len(recv), dt
+
+
+def run_reference(args, w):
+    """--impl reference: the oracle on a bounded sample per step."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import celes_oracle as orc
+    from paper_1706_02145_b200 import workloads
+    pos, rad = workloads.positions(w)
+    b = workloads.gaussian_coefficients(w.N, w.nmax, w.seed_b)
+    t0 = time.perf_counter()
+    orc.coupling_matvec(pos, w.k, w.lmax, b, receivers=np.array([0]))
+    per_recv = time.perf_counter() - t0
+    cores = max(1, orc.LAST_THREADS)
+    budget = 150.0 / max(1, args.steps + args.warmup)                         # seconds per step
+    n_recv = int(max(cores, min(w.N, budget / max(per_recv, 1e-9) * cores)))
+    n_recv = max(cores, (n_recv // cores) * cores)
+    recv = workloads.sample_receivers(w.N, n_recv, 404)
+    for _ in range(args.warmup):
+        orc.coupling_matvec(pos, w.k, w.lmax, b, receivers=recv)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        orc.coupling_matvec(pos, w.k, w.lmax, b, receivers=recv)
+    dt = (time.perf_counter() - t0) / max(1, args.steps)
+    value = len(recv) * (w.N - 1) / dt
+    sample = f"{len(recv)} seeded receivers x {w.N - 1} emitters per step (full emitter sum each)"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"{w.name}: N={w.N} lmax={w.lmax} slab RSA ff=0.3 (sampled receivers)"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+def main():
+    args = parse()
+    from paper_1706_02145_b200 import workloads
+    w = workloads.CONFIGS[args.workload]
+    if args.impl == "reference":
+        run_reference(args, w)
+        return
+
+    import torch
+    import torch.distributed as dist
+    import paper_1706_02145_b200 as celes
+    from paper_1706_02145_b200 import fields
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    pos, rad = workloads.positions(w)
+    q = fields.mie_coefficients(w.lmax, w.k, rad, workloads.N_SPHERE)
+    b_host = workloads.gaussian_coefficients(w.N, w.nmax, w.seed_b + rank)
+    t0 = time.perf_counter()
+    ctx = celes.celes_setup(pos, rad, q, w.k, w.lmax)
+    setup_s = time.perf_counter() - t0
+    cfg = celes.celes_launch_config(ctx)
+    b = torch.from_numpy(b_host).cuda()
+    y = torch.empty_like(b)
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")   # > 126 MB L2
+    stream = torch.cuda.current_stream()
+    pairs = w.N * (w.N - 1)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # FP32 peak of this GPU at its clocks of the moment (FFMA-only probe)
+    probe = {v: celes.celes_fp32_peak_probe(v, 2048)["flops_per_s"] for v in (0, 1, 2)}
+    for _ in range(args.warmup):
+        celes.celes_coupling_matvec(ctx, b, y)
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    barrier()
+    for s in range(args.steps):
+        flush.zero_()                                   # L2 flush between timed iterations (outside the events)
+        ev[s][0].record(stream)
+        celes.celes_coupling_matvec(ctx, b, y)
+        ev[s][1].record(stream)
+    barrier()
+    clocks = sampler.stop()
+    step_ms = [a.elapsed_time(c) for a, c in ev]
+    total_ms = float(sum(step_ms))
+    t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    total_ms = float(t.item())
+    ms_per_step = total_ms / args.steps
+    value = world * pairs * args.steps / (total_ms * 1e-3)
+
+    # end to end: pinned host buffers through the C ABI's host entry point, copies inside the timed region
+    bh = torch.from_numpy(b_host).pin_memory()
+    yh = torch.empty_like(bh).pin_memory()
+    bh_np, yh_np = bh.numpy(), yh.numpy()
+    celes.celes_coupling_matvec_host(ctx, bh_np, yh_np)
+    barrier()
+    t0 = time.perf_counter()
+    for s in range(args.steps):
+        celes.celes_coupling_matvec_host(ctx, bh_np, yh_np)
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    te = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(te, op=dist.ReduceOp.MAX)
+    e2e_value = world * pairs * args.steps / float(te.item())
+
+    if rank == 0:
+        peaks = measured_peaks()
+        sm_count = torch.cuda.get_device_properties(local).multi_processor_count
+        sm_mhz = clocks.get("sm_mhz") or peaks.get("sm_max_mhz") or 1965.0
+        nominal_peak = 2.0 * FP32_LANES_PER_SM * sm_count * (clocks.get("sm_max_mhz") or 1965.0) * 1e6
+        peak_at_clock = 2.0 * FP32_LANES_PER_SM * sm_count * sm_mhz * 1e6
+        flops = FLOPS_PER_PAIR.get(w.lmax, 0.0) * pairs
+        achieved = flops / (ms_per_step * 1e-3)
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": f"{w.name}: N={w.N} lmax={w.lmax} R=100nm n=1.52 lambda=550nm slab RSA ff=0.3",
+                       "pairs_per_step": pairs, "l2": "flushed between timed iterations (256 MiB write)",
+                       "launch": cfg, "parallelism": "replicas only" if world > 1 else "single GPU",
+                       "setup_s": setup_s, "step_ms_min": float(min(step_ms)), "step_ms_median": float(np.median(step_ms))},
+            "clocks": clocks,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(b_host.nbytes),
+                    "d2h_bytes_per_step": int(b_host.nbytes)},
+            "gpu_launches": 3 * args.steps,
+            "roofline": {"bound": "alu", "achieved": achieved / 1e12, "peak": nominal_peak / 1e12, "unit": "TFLOP/s",
+                         "frac": achieved / nominal_peak, "traffic": None,
+                         "peak_kind": "derived: 2 x 128 FP32 lanes x SMs x clocks.max.sm (DESIGN.md section 7)",
+                         "frac_of_peak_at_observed_clock": achieved / peak_at_clock,
+                         "ffma_probe_tflops": {"reg": probe[0] / 1e12, "imm": probe[1] / 1e12, "f32x2": probe[2] / 1e12},
+                         "frac_of_ffma_probe": achieved / max(probe.values()),
+                         "flops_per_pair": FLOPS_PER_PAIR.get(w.lmax)},
+        }
+        if not args.no_cpu_baseline and world == 1:
+            rate, cores, n_recv, dt = oracle_sample_rate(w, pos, b_host, args.cpu_seconds)
+            line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                    "sample": f"{n_recv} seeded receivers x {w.N - 1} emitters ({dt:.1f} s)"}
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

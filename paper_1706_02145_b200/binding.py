@@ -1,0 +1,237 @@
+"""Thin Python binding of the C ABI in include/celes.h: argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels of libceles.so; PyTorch is used for device memory and
+streams.  There is no CPU fallback: a missing library raises ImportError-like RuntimeError at first use, and
+a missing GPU makes celes_setup raise CelesError(CELES_ECUDA).
+
+Function names and semantics are those of include/celes.h (which cites the paper passage for each).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libceles.so")
+
+CELES_OK, CELES_EINVAL, CELES_ENOMEM, CELES_ECUDA, CELES_ENOCONV = 0, -1, -2, -3, -4
+CELES_GMRES = 0
+CELES_MAX_HISTORY = 4096
+EXPORTS = ["celes_setup", "celes_coupling_matvec", "celes_system_matvec", "celes_coupling_matvec_host",
+           "celes_system_matvec_host", "celes_solve", "celes_destroy", "celes_strerror", "celes_nmax",
+           "celes_launch_config", "celes_translation_table", "celes_fp32_peak_probe"]
+
+
+class CelesError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        self.code = code
+        super().__init__(f"{where}: {strerror(code)} ({code})")
+
+
+class celes_options(ctypes.Structure):
+    _fields_ = [("emitter_tile", ctypes.c_int), ("emitter_splits", ctypes.c_int), ("skip_overlap_check", ctypes.c_int)]
+
+
+class celes_solve_opts(ctypes.Structure):
+    _fields_ = [("method", ctypes.c_int), ("restart", ctypes.c_int), ("rtol", ctypes.c_double),
+                ("max_iters", ctypes.c_int)]
+
+
+class celes_solve_info(ctypes.Structure):
+    _fields_ = [("iterations", ctypes.c_int), ("matvecs", ctypes.c_int), ("converged", ctypes.c_int),
+                ("rel_residual", ctypes.c_double), ("seconds", ctypes.c_double), ("n_history", ctypes.c_int),
+                ("history", ctypes.c_double * CELES_MAX_HISTORY)]
+
+
+_LIB = None
+
+
+def lib() -> ctypes.CDLL:
+    """The loaded libceles.so (fails loudly if it has not been built: run `python -m paper_1706_02145_b200.build`)."""
+    global _LIB
+    if _LIB is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"{LIB_PATH} is missing: build it with `python -m paper_1706_02145_b200.build` "
+                               "(there is no CPU fallback)")
+        L = ctypes.CDLL(LIB_PATH)
+        i, d, p = ctypes.c_int, ctypes.c_double, ctypes.c_void_p
+        L.celes_setup.restype = i
+        L.celes_setup.argtypes = [ctypes.POINTER(p), i, i, p, p, p, d, ctypes.POINTER(celes_options), p]
+        for name in ("celes_coupling_matvec", "celes_system_matvec", "celes_coupling_matvec_host",
+                     "celes_system_matvec_host"):
+            getattr(L, name).restype = i
+            getattr(L, name).argtypes = [p, p, p, p]
+        L.celes_solve.restype = i
+        L.celes_solve.argtypes = [p, p, p, ctypes.POINTER(celes_solve_opts), ctypes.POINTER(celes_solve_info), p]
+        L.celes_destroy.restype = None
+        L.celes_destroy.argtypes = [p]
+        L.celes_strerror.restype = ctypes.c_char_p
+        L.celes_strerror.argtypes = [i]
+        L.celes_nmax.restype = i
+        L.celes_nmax.argtypes = [i]
+        L.celes_launch_config.restype = i
+        L.celes_launch_config.argtypes = [p] + [ctypes.POINTER(i)] * 4
+        L.celes_translation_table.restype = i
+        L.celes_translation_table.argtypes = [i, p, p]
+        L.celes_fp32_peak_probe.restype = i
+        L.celes_fp32_peak_probe.argtypes = [i, i, ctypes.POINTER(d), ctypes.POINTER(d), p]
+        _LIB = L
+    return _LIB
+
+
+def strerror(code: int) -> str:
+    return lib().celes_strerror(code).decode()
+
+
+def celes_nmax(lmax: int) -> int:
+    n = lib().celes_nmax(lmax)
+    if n < 0:
+        raise CelesError(n, "celes_nmax")
+    return n
+
+
+def _stream(stream) -> int:
+    if stream is None:
+        import torch
+        return torch.cuda.current_stream().cuda_stream
+    return int(getattr(stream, "cuda_stream", stream))
+
+
+def _check_vec(t, ctx, name):
+    import torch
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.complex64 and t.is_contiguous()
+            and t.numel() == ctx.N * ctx.nmax):
+        raise ValueError(f"{name}: need a contiguous CUDA complex64 tensor with {ctx.N * ctx.nmax} elements")
+
+
+class Context:
+    """Owner of a celes_ctx*; destroyed with the object (or explicitly with celes_destroy)."""
+
+    def __init__(self, handle: int, N: int, lmax: int):
+        self.handle, self.N, self.lmax, self.nmax = handle, N, lmax, celes_nmax(lmax)
+
+    def __del__(self):
+        celes_destroy(self)
+
+
+def celes_setup(pos_xyz, radii, mie_q, k: float, lmax: int, *, emitter_tile: int = 0, emitter_splits: int = 0,
+                skip_overlap_check: bool = False, stream=None) -> Context:
+    """celes_setup of include/celes.h.  pos_xyz [N,3] float64, radii [N] float64, mie_q [N,2,lmax] complex128 (host)."""
+    pos = np.ascontiguousarray(pos_xyz, dtype=np.float64)
+    rad = np.ascontiguousarray(radii, dtype=np.float64)
+    q = np.ascontiguousarray(mie_q, dtype=np.complex128)
+    N = pos.shape[0] if pos.ndim == 2 else 0
+    if pos.ndim != 2 or pos.shape[1] != 3 or rad.shape != (N,) or q.shape != (N, 2, lmax):
+        raise ValueError("celes_setup: pos_xyz [N,3], radii [N], mie_q [N,2,lmax] expected")
+    opt = celes_options(int(emitter_tile), int(emitter_splits), int(bool(skip_overlap_check)))
+    h = ctypes.c_void_p()
+    import torch
+    s = _stream(stream) if torch.cuda.is_available() else 0
+    rc = lib().celes_setup(ctypes.byref(h), N, int(lmax), pos.ctypes.data, rad.ctypes.data, q.ctypes.data,
+                           float(k), ctypes.byref(opt), s)
+    if rc != CELES_OK:
+        raise CelesError(rc, "celes_setup")
+    return Context(h.value, N, int(lmax))
+
+
+def celes_destroy(ctx: Context) -> None:
+    if getattr(ctx, "handle", None):
+        lib().celes_destroy(ctx.handle)
+        ctx.handle = None
+
+
+def celes_coupling_matvec(ctx: Context, b, y=None, stream=None):
+    """y = W b (device tensors, complex64 [N,nmax]); asynchronous on the stream."""
+    import torch
+    _check_vec(b, ctx, "b")
+    if y is None:
+        y = torch.empty_like(b)
+    _check_vec(y, ctx, "y")
+    rc = lib().celes_coupling_matvec(ctx.handle, b.data_ptr(), y.data_ptr(), _stream(stream))
+    if rc != CELES_OK:
+        raise CelesError(rc, "celes_coupling_matvec")
+    return y
+
+
+def celes_system_matvec(ctx: Context, b, out=None, stream=None):
+    """out = b - T (W b) (device tensors); asynchronous on the stream."""
+    import torch
+    _check_vec(b, ctx, "b")
+    if out is None:
+        out = torch.empty_like(b)
+    _check_vec(out, ctx, "out")
+    rc = lib().celes_system_matvec(ctx.handle, b.data_ptr(), out.data_ptr(), _stream(stream))
+    if rc != CELES_OK:
+        raise CelesError(rc, "celes_system_matvec")
+    return out
+
+
+def _host_vec(a, ctx, name):
+    if not (isinstance(a, np.ndarray) and a.dtype == np.complex64 and a.flags.c_contiguous and a.size == ctx.N * ctx.nmax):
+        raise ValueError(f"{name}: need a C-contiguous complex64 ndarray with {ctx.N * ctx.nmax} elements")
+
+
+def celes_coupling_matvec_host(ctx: Context, b_host: np.ndarray, y_host: np.ndarray | None = None, stream=None):
+    """y = W b with HOST buffers (numpy complex64, ideally backed by pinned memory); synchronous."""
+    _host_vec(b_host, ctx, "b_host")
+    if y_host is None:
+        y_host = np.empty_like(b_host)
+    _host_vec(y_host, ctx, "y_host")
+    rc = lib().celes_coupling_matvec_host(ctx.handle, b_host.ctypes.data, y_host.ctypes.data, _stream(stream))
+    if rc != CELES_OK:
+        raise CelesError(rc, "celes_coupling_matvec_host")
+    return y_host
+
+
+def celes_system_matvec_host(ctx: Context, b_host: np.ndarray, out_host: np.ndarray | None = None, stream=None):
+    _host_vec(b_host, ctx, "b_host")
+    if out_host is None:
+        out_host = np.empty_like(b_host)
+    _host_vec(out_host, ctx, "out_host")
+    rc = lib().celes_system_matvec_host(ctx.handle, b_host.ctypes.data, out_host.ctypes.data, _stream(stream))
+    if rc != CELES_OK:
+        raise CelesError(rc, "celes_system_matvec_host")
+    return out_host
+
+
+def celes_solve(ctx: Context, a_in, x, *, restart: int = 30, rtol: float = 1e-4, max_iters: int = 1000, stream=None):
+    """Solve eq. (8) in place in x (in: x0, out: b).  Returns a dict with the celes_solve_info fields; raises
+    CelesError on failure other than CELES_ENOCONV (reported as converged = 0)."""
+    _check_vec(a_in, ctx, "a_in")
+    _check_vec(x, ctx, "x")
+    o = celes_solve_opts(CELES_GMRES, int(restart), float(rtol), int(max_iters))
+    info = celes_solve_info()
+    rc = lib().celes_solve(ctx.handle, a_in.data_ptr(), x.data_ptr(), ctypes.byref(o), ctypes.byref(info), _stream(stream))
+    if rc not in (CELES_OK, CELES_ENOCONV):
+        raise CelesError(rc, "celes_solve")
+    return {"iterations": info.iterations, "matvecs": info.matvecs, "converged": bool(info.converged),
+            "rel_residual": info.rel_residual, "seconds": info.seconds,
+            "history": [info.history[i] for i in range(info.n_history)], "code": rc}
+
+
+def celes_launch_config(ctx: Context) -> dict:
+    v = [ctypes.c_int() for _ in range(4)]
+    rc = lib().celes_launch_config(ctx.handle, *[ctypes.byref(x) for x in v])
+    if rc != CELES_OK:
+        raise CelesError(rc, "celes_launch_config")
+    return dict(zip(("receiver_blocks", "emitter_splits", "block_threads", "emitter_tile"), (x.value for x in v)))
+
+
+def celes_translation_table(lmax: int):
+    """(a5_re, b5_im) [H,H,P] float64 as the library evaluates them on the host (needs no GPU)."""
+    H, P = lmax * (lmax + 2), 2 * lmax + 1
+    a = np.zeros((H, H, P)); b = np.zeros((H, H, P))
+    rc = lib().celes_translation_table(int(lmax), a.ctypes.data, b.ctypes.data)
+    if rc != CELES_OK:
+        raise CelesError(rc, "celes_translation_table")
+    return a, b
+
+
+def celes_fp32_peak_probe(variant: int = 0, iters: int = 4096, stream=None) -> dict:
+    f, ms = ctypes.c_double(), ctypes.c_double()
+    rc = lib().celes_fp32_peak_probe(int(variant), int(iters), ctypes.byref(f), ctypes.byref(ms), _stream(stream))
+    if rc != CELES_OK:
+        raise CelesError(rc, "celes_fp32_peak_probe")
+    return {"flops_per_s": f.value, "ms": ms.value}

@@ -1,0 +1,46 @@
+"""Build step of the CUDA library: nvcc -> paper_1706_02145_b200/libceles.so (in-tree, sm_100a only).
+
+    python -m paper_1706_02145_b200.build [--force] [--regen]
+
+``--regen`` re-runs csrc/gen_coupling_body.py first (needs SymPy; the generated files are committed).
+nvcc cross-compiles without a GPU.  The library is loaded by ``paper_1706_02145_b200.binding`` via ctypes.
+"""
+from __future__ import annotations
+
+import os
+import subprocess
+import sys
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+CSRC = os.path.join(HERE, "csrc")
+LIB = os.path.join(HERE, "libceles.so")
+NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
+              "-shared", "-Xcompiler", "-fPIC"]
+
+
+def sources() -> list[str]:
+    out = [os.path.join(HERE, "..", "include", "celes.h")]
+    for root, _, files in os.walk(CSRC):
+        out += [os.path.join(root, f) for f in files if f.endswith((".cu", ".cuh", ".h", ".inc"))]
+    return out
+
+
+def stale() -> bool:
+    if not os.path.exists(LIB):
+        return True
+    t = os.path.getmtime(LIB)
+    return any(os.path.getmtime(s) > t for s in sources())
+
+
+def build(force: bool = False, regen: bool = False, verbose: bool = False) -> str:
+    if regen:
+        subprocess.run([sys.executable, os.path.join(CSRC, "gen_coupling_body.py")], check=True)
+    if force or stale():
+        nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+        cmd = [nvcc, *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []), "-o", LIB, os.path.join(CSRC, "celes.cu")]
+        subprocess.run(cmd, check=True)
+    return LIB
+
+
+if __name__ == "__main__":
+    print(build(force="--force" in sys.argv, regen="--regen" in sys.argv, verbose="-v" in sys.argv))

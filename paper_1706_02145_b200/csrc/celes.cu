@@ -1,0 +1,557 @@
+// celes.cu -- C-ABI library of the B200-native CELES hot path (include/celes.h).
+//
+// Host side of the boundary: argument validation, context (device tables + work space), kernel launches for
+// y = W b (eq. 6-7) and out = b - T (W b) (eq. 8-9), and the host-driven
+// restarted GMRES of celes_solve whose vector work is device kernels (krylov_kernels.cuh).
+// Nothing here falls back to the CPU: without a device every compute entry point returns CELES_ECUDA.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <chrono>
+#include <cmath>
+#include <complex>
+#include <cstdint>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/celes.h"
+#include "coupling_kernel.cuh"
+#include "krylov_kernels.cuh"
+#include "translation_table.h"
+
+struct celes_ctx {
+    int N = 0, lmax = 0, nmax = 0;
+    double k = 0.0;
+    int device = 0, sm_count = 0;
+    int rblocks = 0, splits = 1, chunk = 0, etile = 32;
+    size_t coupling_smem = 0;
+    double* kpos = nullptr;      // [N][3] FP64, k * r_i
+    float2* tdiag = nullptr;     // [N][nmax] T diagonal Q^i_{tau,l} expanded over m (B.1)
+    float2* bpm = nullptr;       // [N][nmax] work: [b_+ | b_-]
+    float2* ypart = nullptr;     // [splits][N][nmax] work: partial sums of the emitter splits
+    // Krylov work space (allocated on the first celes_solve)
+    int kry_restart = 0, dot_blocks = 0;
+    float2* V = nullptr;         // [restart+1][n] basis
+    float2* rhs = nullptr;       // [n] T a_in
+    float2* tmp = nullptr;       // [n]
+    double2* partial = nullptr;  // [dot_blocks][restart+1]
+    double2* coef = nullptr;     // [restart+2]
+    double2* hsum = nullptr;     // [restart+2]
+    double2* hhost = nullptr;    // pinned [restart+2]
+};
+
+namespace {
+
+using celes::kBlock;
+
+#define CU_TRY(expr)                                  \
+    do {                                              \
+        cudaError_t e_ = (expr);                      \
+        if (e_ != cudaSuccess) {                      \
+            return e_ == cudaErrorMemoryAllocation ? CELES_ENOMEM : CELES_ECUDA; \
+        }                                             \
+    } while (0)
+
+template <int LMAX>
+int launch_coupling_t(const celes_ctx* c, cudaStream_t s) {
+    const size_t smem = celes::coupling_smem_bytes<LMAX>(c->etile);
+    dim3 grid(c->rblocks, c->splits);
+    celes::coupling_kernel<LMAX><<<grid, kBlock, smem, s>>>(c->N, c->chunk, c->etile, c->kpos, c->bpm, c->ypart);
+    return cudaGetLastError() == cudaSuccess ? CELES_OK : CELES_ECUDA;
+}
+
+template <int LMAX>
+int prepare_coupling_t(celes_ctx* c) {
+    const size_t smem = celes::coupling_smem_bytes<LMAX>(c->etile);
+    c->coupling_smem = smem;
+    CU_TRY(cudaFuncSetAttribute(celes::coupling_kernel<LMAX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    return CELES_OK;
+}
+
+template <int LMAX>
+int occupancy_t(const celes_ctx* c, int* ctas_per_sm) {
+    CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, celes::coupling_kernel<LMAX>, kBlock,
+                                                         celes::coupling_smem_bytes<LMAX>(c->etile)));
+    return CELES_OK;
+}
+
+int launch_coupling(const celes_ctx* c, cudaStream_t s) {
+    switch (c->lmax) {
+        case 1: return launch_coupling_t<1>(c, s);
+        case 2: return launch_coupling_t<2>(c, s);
+        case 3: return launch_coupling_t<3>(c, s);
+        case 4: return launch_coupling_t<4>(c, s);
+    }
+    return CELES_EINVAL;
+}
+
+int prepare_coupling(celes_ctx* c, int* ctas_per_sm) {
+    int rc = CELES_EINVAL;
+    switch (c->lmax) {
+        case 1: rc = prepare_coupling_t<1>(c); if (!rc) rc = occupancy_t<1>(c, ctas_per_sm); break;
+        case 2: rc = prepare_coupling_t<2>(c); if (!rc) rc = occupancy_t<2>(c, ctas_per_sm); break;
+        case 3: rc = prepare_coupling_t<3>(c); if (!rc) rc = occupancy_t<3>(c, ctas_per_sm); break;
+        case 4: rc = prepare_coupling_t<4>(c); if (!rc) rc = occupancy_t<4>(c, ctas_per_sm); break;
+    }
+    return rc;
+}
+
+// y = W b (tdiag == nullptr) or out = b - T (W b): pack -> coupling -> finalize, all on stream s.
+int run_matvec(celes_ctx* c, const float2* b, float2* out, bool system, cudaStream_t s) {
+    const int H = c->nmax / 2;
+    const long long nh = (long long)c->N * H;
+    const int tb = 256;
+    const unsigned gb = (unsigned)((nh + tb - 1) / tb);
+    celes::pack_kernel<<<gb, tb, 0, s>>>(c->N, H, b, c->bpm);
+    if (cudaGetLastError() != cudaSuccess) return CELES_ECUDA;
+    int rc = launch_coupling(c, s);
+    if (rc) return rc;
+    celes::finalize_kernel<<<gb, tb, 0, s>>>(c->N, H, c->splits, c->ypart, system ? c->tdiag : nullptr, b, out);
+    return cudaGetLastError() == cudaSuccess ? CELES_OK : CELES_ECUDA;
+}
+
+// Spheres must be disjoint ((A.5) needs |r| < |d|).  Uniform grid of cell edge 2 Rmax: every
+// sphere is compared with the spheres of the 27 cells around it.  O(N log N).
+bool spheres_disjoint(int N, const double* pos, const double* rad) {
+    if (N < 2) return true;
+    double rmax = 0.0, lo[3] = {pos[0], pos[1], pos[2]};
+    for (int i = 0; i < N; ++i) {
+        rmax = std::max(rmax, rad[i]);
+        for (int a = 0; a < 3; ++a) lo[a] = std::min(lo[a], pos[3 * i + a]);
+    }
+    const double cell = std::max(2.0 * rmax, 1e-300);
+    struct Key { int64_t c[3]; int i; };
+    std::vector<Key> keys(N);
+    for (int i = 0; i < N; ++i) {
+        for (int a = 0; a < 3; ++a) keys[i].c[a] = (int64_t)std::floor((pos[3 * i + a] - lo[a]) / cell);
+        keys[i].i = i;
+    }
+    auto less = [](const Key& x, const Key& y) {
+        if (x.c[0] != y.c[0]) return x.c[0] < y.c[0];
+        if (x.c[1] != y.c[1]) return x.c[1] < y.c[1];
+        return x.c[2] < y.c[2];
+    };
+    std::sort(keys.begin(), keys.end(), less);
+    for (int a = 0; a < N; ++a) {
+        const Key& ka = keys[a];
+        for (int64_t dx = -1; dx <= 1; ++dx)
+            for (int64_t dy = -1; dy <= 1; ++dy) {
+                // the three z-neighbours of (cx+dx, cy+dy) are contiguous in the sorted order
+                Key probe{{ka.c[0] + dx, ka.c[1] + dy, ka.c[2] - 1}, 0};
+                auto it = std::lower_bound(keys.begin(), keys.end(), probe, less);
+                for (; it != keys.end() && it->c[0] == probe.c[0] && it->c[1] == probe.c[1] && it->c[2] <= ka.c[2] + 1; ++it) {
+                    const int i = ka.i, j = it->i;
+                    if (j <= i) continue;
+                    const double ex = pos[3 * i] - pos[3 * j], ey = pos[3 * i + 1] - pos[3 * j + 1],
+                                 ez = pos[3 * i + 2] - pos[3 * j + 2];
+                    const double rr = rad[i] + rad[j];
+                    if (ex * ex + ey * ey + ez * ez < rr * rr) return false;
+                }
+            }
+    }
+    return true;
+}
+
+void free_ctx(celes_ctx* c) {
+    if (!c) return;
+    cudaFree(c->kpos); cudaFree(c->tdiag); cudaFree(c->bpm); cudaFree(c->ypart);
+    cudaFree(c->V); cudaFree(c->rhs); cudaFree(c->tmp); cudaFree(c->partial); cudaFree(c->coef); cudaFree(c->hsum);
+    if (c->hhost) cudaFreeHost(c->hhost);
+    delete c;
+}
+
+int ensure_krylov(celes_ctx* c, int restart) {
+    if (c->V && c->kry_restart >= restart) return CELES_OK;
+    cudaFree(c->V); cudaFree(c->rhs); cudaFree(c->tmp); cudaFree(c->partial); cudaFree(c->coef); cudaFree(c->hsum);
+    if (c->hhost) cudaFreeHost(c->hhost);
+    c->V = nullptr; c->rhs = c->tmp = nullptr; c->partial = c->coef = c->hsum = nullptr; c->hhost = nullptr;
+    const size_t n = (size_t)c->N * c->nmax;
+    c->dot_blocks = (int)std::min<size_t>((n + celes::kDotBlock - 1) / celes::kDotBlock, (size_t)c->sm_count * 4);
+    CU_TRY(cudaMalloc(&c->V, sizeof(float2) * n * (restart + 1)));
+    CU_TRY(cudaMalloc(&c->rhs, sizeof(float2) * n));
+    CU_TRY(cudaMalloc(&c->tmp, sizeof(float2) * n));
+    CU_TRY(cudaMalloc(&c->partial, sizeof(double2) * c->dot_blocks * (restart + 1)));
+    CU_TRY(cudaMalloc(&c->coef, sizeof(double2) * (restart + 2)));
+    CU_TRY(cudaMalloc(&c->hsum, sizeof(double2) * (restart + 2)));
+    CU_TRY(cudaMallocHost(&c->hhost, sizeof(double2) * (restart + 2)));
+    c->kry_restart = restart;
+    return CELES_OK;
+}
+
+// out[0..k) (device) = V[0..k)^H w; optionally accumulated into accum.
+int device_dots(celes_ctx* c, long long n, int k, const float2* V, const float2* w, double2* out, double2* accum,
+                cudaStream_t s) {
+    celes::multi_dot_kernel<<<c->dot_blocks, celes::kDotBlock, 0, s>>>(n, k, V, w, c->partial);
+    celes::dots_reduce_kernel<<<(k + 63) / 64, 64, 0, s>>>(c->dot_blocks, k, c->partial, out, accum);
+    return cudaGetLastError() == cudaSuccess ? CELES_OK : CELES_ECUDA;
+}
+
+int device_axpys(celes_ctx* c, long long n, int k, double alpha, const double2* coef, const float2* V, float2* w,
+                 cudaStream_t s) {
+    const int blocks = (int)std::min<long long>((n + 255) / 256, (long long)c->sm_count * 8);
+    celes::multi_axpy_kernel<<<blocks, 256, sizeof(double2) * k, s>>>(n, k, alpha, coef, V, w);
+    return cudaGetLastError() == cudaSuccess ? CELES_OK : CELES_ECUDA;
+}
+
+// ||v||_2 on the host (synchronises s)
+int device_norm(celes_ctx* c, long long n, const float2* v, double* out, cudaStream_t s) {
+    int rc = device_dots(c, n, 1, v, v, c->coef, nullptr, s);
+    if (rc) return rc;
+    CU_TRY(cudaMemcpyAsync(c->hhost, c->coef, sizeof(double2), cudaMemcpyDeviceToHost, s));
+    CU_TRY(cudaStreamSynchronize(s));
+    *out = std::sqrt(std::max(0.0, c->hhost[0].x));
+    return CELES_OK;
+}
+
+// ---- FP32 peak probe kernels -----------------------------------------------------------------------------
+template <int VARIANT>
+__global__ void __launch_bounds__(256) ffma_probe_kernel(int iters, float seed, float* sink) {
+    constexpr int C = 16;                         // independent chains per thread
+    float a[C];
+#pragma unroll
+    for (int c = 0; c < C; ++c) a[c] = seed + (float)(threadIdx.x + c);
+    const float m = 0.999f + seed * 1e-9f, d = seed * 1e-3f;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            if (VARIANT == 0) {
+#pragma unroll
+                for (int c = 0; c < C; ++c) a[c] = fmaf(a[c], m, d);
+            } else if (VARIANT == 1) {
+#pragma unroll
+                for (int c = 0; c < C; ++c) a[c] = fmaf(a[c], 0.99951171875f, d);
+            } else {
+#pragma unroll
+                for (int c = 0; c < C; c += 2) {
+                    unsigned long long acc, mm, dd;
+                    asm("mov.b64 %0, {%1, %2};" : "=l"(acc) : "f"(a[c]), "f"(a[c + 1]));
+                    asm("mov.b64 %0, {%1, %1};" : "=l"(mm) : "f"(m));
+                    asm("mov.b64 %0, {%1, %1};" : "=l"(dd) : "f"(d));
+                    asm("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(acc) : "l"(mm), "l"(dd));
+                    asm("mov.b64 {%0, %1}, %2;" : "=f"(a[c]), "=f"(a[c + 1]) : "l"(acc));
+                }
+            }
+        }
+    }
+    float t = 0.f;
+#pragma unroll
+    for (int c = 0; c < C; ++c) t += a[c];
+    if (t == 12345.678f) sink[0] = t;             // never true in practice; keeps the chains alive
+}
+
+}  // namespace
+
+// ---------------------------------------------------------------------------------------------------------
+extern "C" {
+
+int celes_nmax(int lmax) {
+    if (lmax < CELES_LMAX_MIN || lmax > CELES_LMAX_MAX) return CELES_EINVAL;
+    return 2 * lmax * (lmax + 2);
+}
+
+const char* celes_strerror(int code) {
+    switch (code) {
+        case CELES_OK: return "success";
+        case CELES_EINVAL: return "invalid argument";
+        case CELES_ENOMEM: return "out of memory";
+        case CELES_ECUDA: return "CUDA error or no CUDA device";
+        case CELES_ENOCONV: return "iterative solver did not converge within max_iters";
+    }
+    return "unknown error code";
+}
+
+int celes_translation_table(int lmax, double* a5_re, double* b5_im) {
+    if (lmax < CELES_LMAX_MIN || lmax > CELES_LMAX_MAX || !a5_re || !b5_im) return CELES_EINVAL;
+    std::vector<double> a, b;
+    if (!celes::build_translation_table(lmax, a, b)) return CELES_EINVAL;
+    std::memcpy(a5_re, a.data(), sizeof(double) * a.size());
+    std::memcpy(b5_im, b.data(), sizeof(double) * b.size());
+    return CELES_OK;
+}
+
+int celes_setup(celes_ctx** out, int N, int lmax, const double* pos_xyz, const double* radii, const double* mie_q,
+                double k, const celes_options* opt, void* cuda_stream) {
+    if (!out) return CELES_EINVAL;
+    *out = nullptr;
+    if (N < 1 || lmax < CELES_LMAX_MIN || lmax > CELES_LMAX_MAX || !pos_xyz || !radii || !mie_q) return CELES_EINVAL;
+    if (!(k > 0.0) || !std::isfinite(k)) return CELES_EINVAL;
+    if ((long long)N * celes_nmax(lmax) > (1LL << 31)) return CELES_EINVAL;
+    const int nmax = celes_nmax(lmax), H = nmax / 2;
+    for (long long t = 0; t < 3LL * N; ++t) if (!std::isfinite(pos_xyz[t])) return CELES_EINVAL;
+    for (int i = 0; i < N; ++i) if (!std::isfinite(radii[i]) || !(radii[i] > 0.0)) return CELES_EINVAL;
+    for (long long t = 0; t < 4LL * N * lmax; ++t) if (!std::isfinite(mie_q[t])) return CELES_EINVAL;
+    const bool skip = opt && opt->skip_overlap_check;
+    if (!skip && !spheres_disjoint(N, pos_xyz, radii)) return CELES_EINVAL;
+    if (opt && (opt->emitter_tile < 0 || opt->emitter_splits < 0 || opt->emitter_tile > 128)) return CELES_EINVAL;
+
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); return CELES_ECUDA; }
+    celes_ctx* c = new (std::nothrow) celes_ctx;
+    if (!c) return CELES_ENOMEM;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    c->N = N; c->lmax = lmax; c->nmax = nmax; c->k = k;
+    int rc = CELES_OK;
+    auto fail = [&](int code) { free_ctx(c); return code; };
+    if (cudaGetDevice(&c->device) != cudaSuccess) return fail(CELES_ECUDA);
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, c->device) != cudaSuccess) return fail(CELES_ECUDA);
+    c->sm_count = prop.multiProcessorCount;
+    c->etile = (opt && opt->emitter_tile > 0) ? opt->emitter_tile : 32;
+    c->rblocks = (N + kBlock - 1) / kBlock;
+    int ctas_per_sm = 1;
+    rc = prepare_coupling(c, &ctas_per_sm);
+    if (rc) return fail(rc);
+    ctas_per_sm = std::max(1, ctas_per_sm);
+    if (opt && opt->emitter_splits > 0) {
+        c->splits = std::min(opt->emitter_splits, N);
+    } else {
+        // Split the emitter sum so that the grid is a whole number of waves (slots = SMs x resident CTAs):
+        // the smallest number of waves that gives every CTA at least ~256 emitters, at most 16 waves.
+        const long long slots = (long long)c->sm_count * ctas_per_sm;
+        long long best = 1;
+        for (long long waves = 1; waves <= 16; ++waves) {
+            long long sp = std::max<long long>(1, (waves * slots) / c->rblocks);
+            if (sp * c->rblocks > waves * slots) continue;
+            best = sp;
+            if ((double)sp * c->rblocks >= 0.9 * waves * slots && waves >= 2) break;
+        }
+        const long long maxsp = std::max<long long>(1, N / 256);
+        c->splits = (int)std::max<long long>(1, std::min<long long>(best, maxsp));
+    }
+    c->chunk = (N + c->splits - 1) / c->splits;
+    c->splits = (N + c->chunk - 1) / c->chunk;
+
+    const size_t n = (size_t)N * nmax;
+    std::vector<double> kp(3 * (size_t)N);
+    for (size_t t = 0; t < kp.size(); ++t) kp[t] = k * pos_xyz[t];
+    std::vector<float2> td(n);
+    const std::complex<double>* q = reinterpret_cast<const std::complex<double>*>(mie_q);
+    for (int i = 0; i < N; ++i)
+        for (int tau = 0; tau < 2; ++tau)
+            for (int l = 1; l <= lmax; ++l)
+                for (int m = -l; m <= l; ++m) {
+                    const std::complex<double> v = q[((size_t)i * 2 + tau) * lmax + (l - 1)];
+                    td[(size_t)i * nmax + tau * H + (l - 1) * (l + 1) + (m + l)] = make_float2((float)v.real(), (float)v.imag());
+                }
+#define SETUP_TRY(expr)                                                        \
+    do {                                                                       \
+        cudaError_t e_ = (expr);                                               \
+        if (e_ != cudaSuccess) return fail(e_ == cudaErrorMemoryAllocation ? CELES_ENOMEM : CELES_ECUDA); \
+    } while (0)
+    SETUP_TRY(cudaMalloc(&c->kpos, sizeof(double) * kp.size()));
+    SETUP_TRY(cudaMalloc(&c->tdiag, sizeof(float2) * n));
+    SETUP_TRY(cudaMalloc(&c->bpm, sizeof(float2) * n));
+    SETUP_TRY(cudaMalloc(&c->ypart, sizeof(float2) * n * c->splits));
+    SETUP_TRY(cudaMemcpyAsync(c->kpos, kp.data(), sizeof(double) * kp.size(), cudaMemcpyHostToDevice, s));
+    SETUP_TRY(cudaMemcpyAsync(c->tdiag, td.data(), sizeof(float2) * n, cudaMemcpyHostToDevice, s));
+    SETUP_TRY(cudaStreamSynchronize(s));
+#undef SETUP_TRY
+    *out = c;
+    return CELES_OK;
+}
+
+int celes_coupling_matvec(celes_ctx* ctx, const void* b_dev, void* y_dev, void* cuda_stream) {
+    if (!ctx || !b_dev || !y_dev || b_dev == y_dev) return CELES_EINVAL;
+    return run_matvec(ctx, (const float2*)b_dev, (float2*)y_dev, false, (cudaStream_t)cuda_stream);
+}
+
+int celes_system_matvec(celes_ctx* ctx, const void* b_dev, void* out_dev, void* cuda_stream) {
+    if (!ctx || !b_dev || !out_dev || b_dev == out_dev) return CELES_EINVAL;
+    return run_matvec(ctx, (const float2*)b_dev, (float2*)out_dev, true, (cudaStream_t)cuda_stream);
+}
+
+static int matvec_host(celes_ctx* ctx, const void* b_host, void* y_host, bool system, void* cuda_stream) {
+    if (!ctx || !b_host || !y_host) return CELES_EINVAL;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const size_t bytes = sizeof(float2) * (size_t)ctx->N * ctx->nmax;
+    float2 *bd = nullptr, *yd = nullptr;
+    CU_TRY(cudaMalloc(&bd, bytes));
+    if (cudaMalloc(&yd, bytes) != cudaSuccess) { cudaFree(bd); return CELES_ENOMEM; }
+    int rc = CELES_OK;
+    if (cudaMemcpyAsync(bd, b_host, bytes, cudaMemcpyHostToDevice, s) != cudaSuccess) rc = CELES_ECUDA;
+    if (!rc) rc = run_matvec(ctx, bd, yd, system, s);
+    if (!rc && cudaMemcpyAsync(y_host, yd, bytes, cudaMemcpyDeviceToHost, s) != cudaSuccess) rc = CELES_ECUDA;
+    if (cudaStreamSynchronize(s) != cudaSuccess && !rc) rc = CELES_ECUDA;
+    cudaFree(bd); cudaFree(yd);
+    return rc;
+}
+
+int celes_coupling_matvec_host(celes_ctx* ctx, const void* b_host, void* y_host, void* cuda_stream) {
+    return matvec_host(ctx, b_host, y_host, false, cuda_stream);
+}
+
+int celes_system_matvec_host(celes_ctx* ctx, const void* b_host, void* out_host, void* cuda_stream) {
+    return matvec_host(ctx, b_host, out_host, true, cuda_stream);
+}
+
+int celes_launch_config(const celes_ctx* ctx, int* receiver_blocks, int* emitter_splits, int* block_threads,
+                        int* emitter_tile) {
+    if (!ctx) return CELES_EINVAL;
+    if (receiver_blocks) *receiver_blocks = ctx->rblocks;
+    if (emitter_splits) *emitter_splits = ctx->splits;
+    if (block_threads) *block_threads = kBlock;
+    if (emitter_tile) *emitter_tile = ctx->etile;
+    return CELES_OK;
+}
+
+// Restarted GMRES (Saad & Schultz, the paper's ref. [26]) on M x = T a_in, unpreconditioned,
+// classical Gram-Schmidt with one re-orthogonalisation pass (CGS2): the j+1 inner products of a pass are ONE
+// kernel, their coefficients stay on the device for the update, and one small device->host copy per inner
+// iteration brings the Hessenberg column to the host, where Givens rotations track the residual estimate.
+// The TRUE residual is recomputed at every restart and decides convergence (reading R14).
+int celes_solve(celes_ctx* ctx, const void* a_in_dev, void* x_dev, const celes_solve_opts* o, celes_solve_info* info,
+                void* cuda_stream) {
+    if (!ctx || !a_in_dev || !x_dev) return CELES_EINVAL;
+    const int method = o ? o->method : CELES_GMRES;
+    const int restart = (o && o->restart > 0) ? o->restart : 30;
+    const double rtol = (o && o->rtol > 0.0) ? o->rtol : 1e-4;
+    const int max_iters = (o && o->max_iters > 0) ? o->max_iters : 1000;
+    if (method != CELES_GMRES || restart > 1024) return CELES_EINVAL;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const auto t_start = std::chrono::steady_clock::now();
+    int rc = ensure_krylov(ctx, restart);
+    if (rc) return rc;
+    const long long n = (long long)ctx->N * ctx->nmax;
+    const int eb = (int)std::min<long long>((n + 255) / 256, (long long)ctx->sm_count * 8);
+    float2* x = (float2*)x_dev;
+    float2* V = ctx->V;
+    typedef std::complex<double> cd;
+
+    int iterations = 0, matvecs = 0, n_hist = 0, converged = 0;
+    double rel = 0.0;
+    if (info) std::memset(info, 0, sizeof(*info));
+    auto push_hist = [&](double v) { if (info && n_hist < CELES_MAX_HISTORY) info->history[n_hist++] = v; };
+    auto finish = [&](int code) {
+        if (info) {
+            info->iterations = iterations; info->matvecs = matvecs; info->converged = converged;
+            info->rel_residual = rel; info->n_history = n_hist;
+            info->seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_start).count();
+        }
+        return code;
+    };
+
+    // rhs = T a_in (eq. 8)
+    celes::tapply_kernel<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(n, ctx->tdiag, (const float2*)a_in_dev, ctx->rhs);
+    double fnorm = 0.0;
+    rc = device_norm(ctx, n, ctx->rhs, &fnorm, s);
+    if (rc) return finish(rc);
+    if (fnorm == 0.0) {                       // zero right-hand side: x = 0
+        CU_TRY(cudaMemsetAsync(x, 0, sizeof(float2) * n, s));
+        CU_TRY(cudaStreamSynchronize(s));
+        converged = 1;
+        return finish(CELES_OK);
+    }
+
+    std::vector<cd> Hm((size_t)(restart + 1) * restart), g(restart + 1), cs(restart), sn(restart), yv(restart);
+    while (true) {
+        // true residual r = rhs - M x  -> V_0
+        rc = run_matvec(ctx, x, ctx->tmp, true, s);
+        if (rc) return finish(rc);
+        ++matvecs;
+        celes::sub_kernel<<<eb, 256, 0, s>>>(n, ctx->rhs, ctx->tmp, V);
+        double beta = 0.0;
+        rc = device_norm(ctx, n, V, &beta, s);
+        if (rc) return finish(rc);
+        rel = beta / fnorm;
+        if (n_hist == 0) push_hist(rel);
+        if (rel <= rtol) { converged = 1; return finish(CELES_OK); }
+        if (iterations >= max_iters) return finish(CELES_ENOCONV);
+        if (!std::isfinite(rel)) return finish(CELES_ECUDA);
+        // V_0 = r / beta  (coef[0] still holds <r,r>)
+        celes::scale_by_inv_norm_kernel<<<eb, 256, 0, s>>>(n, ctx->coef, V, V);
+        std::fill(g.begin(), g.end(), cd(0.0));
+        g[0] = beta;
+        int j = 0;
+        for (; j < restart && iterations < max_iters; ++j) {
+            float2* w = V + (size_t)(j + 1) * n;
+            rc = run_matvec(ctx, V + (size_t)j * n, w, true, s);
+            if (rc) return finish(rc);
+            ++matvecs; ++iterations;
+            CU_TRY(cudaMemsetAsync(ctx->hsum, 0, sizeof(double2) * (j + 2), s));
+            for (int pass = 0; pass < 2; ++pass) {
+                rc = device_dots(ctx, n, j + 1, V, w, ctx->coef, ctx->hsum, s);
+                if (rc) return finish(rc);
+                rc = device_axpys(ctx, n, j + 1, -1.0, ctx->coef, V, w, s);
+                if (rc) return finish(rc);
+            }
+            rc = device_dots(ctx, n, 1, w, w, ctx->hsum + (j + 1), nullptr, s);
+            if (rc) return finish(rc);
+            celes::scale_by_inv_norm_kernel<<<eb, 256, 0, s>>>(n, ctx->hsum + (j + 1), w, w);
+            CU_TRY(cudaMemcpyAsync(ctx->hhost, ctx->hsum, sizeof(double2) * (j + 2), cudaMemcpyDeviceToHost, s));
+            CU_TRY(cudaStreamSynchronize(s));
+            // Hessenberg column j, Givens rotations
+            cd* col = &Hm[(size_t)j * (restart + 1)];
+            for (int i = 0; i <= j; ++i) col[i] = cd(ctx->hhost[i].x, ctx->hhost[i].y);
+            const double hnext = std::sqrt(std::max(0.0, ctx->hhost[j + 1].x));
+            for (int i = 0; i < j; ++i) {
+                const cd t = cs[i] * col[i] + sn[i] * col[i + 1];
+                col[i + 1] = -std::conj(sn[i]) * col[i] + cs[i] * col[i + 1];
+                col[i] = t;
+            }
+            const double denom = std::sqrt(std::norm(col[j]) + hnext * hnext);
+            if (denom == 0.0) break;                               // exact breakdown: drop the column
+            cs[j] = std::abs(col[j]) / denom;                       // real c, complex s (|c|^2 + |s|^2 = 1)
+            const cd phase = (std::abs(col[j]) > 0.0) ? col[j] / std::abs(col[j]) : cd(1.0);
+            sn[j] = phase * hnext / denom;
+            col[j] = phase * denom;
+            g[j + 1] = -std::conj(sn[j]) * g[j];
+            g[j] = cs[j] * g[j];
+            const double est = std::abs(g[j + 1]) / fnorm;
+            push_hist(est);
+            if (est <= rtol || hnext == 0.0) { ++j; break; }
+        }
+        // back substitution R y = g, x += V y
+        for (int i = j - 1; i >= 0; --i) {
+            cd acc = g[i];
+            for (int q = i + 1; q < j; ++q) acc -= Hm[(size_t)q * (restart + 1) + i] * yv[q];
+            yv[i] = acc / Hm[(size_t)i * (restart + 1) + i];
+        }
+        for (int i = 0; i < j; ++i) ctx->hhost[i] = make_double2(yv[i].real(), yv[i].imag());
+        CU_TRY(cudaMemcpyAsync(ctx->coef, ctx->hhost, sizeof(double2) * j, cudaMemcpyHostToDevice, s));
+        if (j > 0) {
+            rc = device_axpys(ctx, n, j, 1.0, ctx->coef, V, x, s);
+            if (rc) return finish(rc);
+        }
+        CU_TRY(cudaStreamSynchronize(s));      // hhost is reused by the next cycle
+    }
+}
+
+void celes_destroy(celes_ctx* ctx) { free_ctx(ctx); }
+
+int celes_fp32_peak_probe(int variant, int iters, double* flops_per_s, double* milliseconds, void* cuda_stream) {
+    if (variant < 0 || variant > 2 || iters < 1) return CELES_EINVAL;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); return CELES_ECUDA; }
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    int dev = 0;
+    cudaDeviceProp prop;
+    CU_TRY(cudaGetDevice(&dev));
+    CU_TRY(cudaGetDeviceProperties(&prop, dev));
+    float* sink = nullptr;
+    CU_TRY(cudaMalloc(&sink, sizeof(float)));
+    const int blocks = prop.multiProcessorCount * 8, threads = 256;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    auto launch = [&](int it) {
+        if (variant == 0) ffma_probe_kernel<0><<<blocks, threads, 0, s>>>(it, 1.0f, sink);
+        else if (variant == 1) ffma_probe_kernel<1><<<blocks, threads, 0, s>>>(it, 1.0f, sink);
+        else ffma_probe_kernel<2><<<blocks, threads, 0, s>>>(it, 1.0f, sink);
+    };
+    launch(std::max(1, iters / 10));              // warm-up
+    cudaEventRecord(e0, s);
+    launch(iters);
+    cudaEventRecord(e1, s);
+    int rc = CELES_OK;
+    if (cudaEventSynchronize(e1) != cudaSuccess || cudaGetLastError() != cudaSuccess) rc = CELES_ECUDA;
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(sink);
+    const double fmas = (double)blocks * threads * 16.0 * 8.0 * (double)iters;
+    if (flops_per_s) *flops_per_s = 2.0 * fmas / (ms * 1e-3);
+    if (milliseconds) *milliseconds = ms;
+    return rc;
+}
+
+}  // extern "C"

@@ -39,7 +39,7 @@ struct YRegs {                       // registers: every index is a literal afte
     }
     __device__ __forceinline__ void operator()(int q, float r, float i) { re[q] += r; im[q] += i; }
     __device__ __forceinline__ float2 get(int q) const { return make_float2(re[q], im[q]); }
-    static constexpr size_t smem_bytes() { return 0; }
+    __host__ __device__ static constexpr size_t smem_bytes() { return 0; }
 };
 
 template <int NMAX>
@@ -56,7 +56,7 @@ struct YSmem {                       // shared memory slab [q][thread] (float2):
         base[q * kBlock] = v;
     }
     __device__ __forceinline__ float2 get(int q) const { return base[q * kBlock]; }
-    static constexpr size_t smem_bytes() { return sizeof(float2) * NMAX * kBlock; }
+    __host__ __device__ static constexpr size_t smem_bytes() { return sizeof(float2) * NMAX * kBlock; }
 };
 
 template <int LMAX>

@@ -1,0 +1,195 @@
+"""GPU parity tests: the CUDA path, called through the C ABI (via the thin binding), against the FP64 oracle
+on the same seeded inputs.  Tolerances are BASELINE.json's: coupling / system matvec relative L2 <= 1e-4,
+solve <= 1e-3 at solver tolerance 1e-4."""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+
+import paper_1706_02145_b200 as celes
+from paper_1706_02145_b200 import fields, workloads
+from oracle import celes_oracle as orc
+
+pytestmark = pytest.mark.gpu
+
+MATVEC_TOL = 1e-4      # BASELINE.json north_star: FP32 vs FP64 coupling matvec
+SOLVE_TOL = 1e-3       # BASELINE.json north_star: solve at solver tolerance 1e-4
+
+
+def rel(a, b):
+    return float(np.linalg.norm(np.asarray(a) - np.asarray(b)) / np.linalg.norm(b))
+
+
+def make(w, **opts):
+    pos, rad = workloads.positions(w)
+    q = fields.mie_coefficients(w.lmax, w.k, rad, workloads.N_SPHERE)
+    ctx = celes.celes_setup(pos, rad, q, w.k, w.lmax, **opts)
+    b = workloads.gaussian_coefficients(w.N, w.nmax, w.seed_b)
+    return pos, rad, q, ctx, b
+
+
+def gpu_coupling(ctx, b):
+    return celes.celes_coupling_matvec(ctx, torch.from_numpy(b).cuda()).cpu().numpy()
+
+
+def test_c1_coupling_system_and_solve():
+    w = workloads.C1
+    pos, rad, q, ctx, b = make(w)
+    ref = orc.coupling_matvec(pos, w.k, w.lmax, b)
+    assert rel(gpu_coupling(ctx, b), ref) <= MATVEC_TOL
+    out = celes.celes_system_matvec(ctx, torch.from_numpy(b).cuda()).cpu().numpy()
+    qo = orc.mie_q(w.lmax, w.k, rad, workloads.N_SPHERE)
+    assert rel(out, orc.system_matvec(pos, w.k, w.lmax, qo, b)) <= MATVEC_TOL
+    a_in = orc.plane_wave_a_in(pos, w.k, w.lmax)
+    x = torch.zeros(w.N, w.nmax, dtype=torch.complex64, device="cuda")
+    info = celes.celes_solve(ctx, torch.from_numpy(a_in.astype(np.complex64)).cuda(), x)
+    assert info["converged"] and info["rel_residual"] <= 1e-4
+    assert rel(x.cpu().numpy(), orc.solve_dense(pos, w.k, w.lmax, qo, a_in)) <= SOLVE_TOL
+
+
+@pytest.mark.parametrize("lmax", [1, 2, 3, 4])
+def test_every_lmax_small_cluster(lmax):
+    w = workloads.Workload(f"L{lmax}", 77, lmax, 90.0, 110.0, "cube", 1800.0, 0.0, 111, 311, 211)
+    pos, rad, q, ctx, b = make(w)
+    assert rel(gpu_coupling(ctx, b), orc.coupling_matvec(pos, w.k, lmax, b)) <= MATVEC_TOL
+
+
+@pytest.mark.parametrize("splits,tile", [(1, 32), (3, 7), (5, 64), (2, 1)])
+def test_ragged_tiles_and_splits(splits, tile):
+    """N not a multiple of the receiver block, the emitter tile or the split chunk."""
+    w = workloads.Workload("ragged", 301, 3, 100.0, 100.0, "cube", 3500.0, 0.0, 112, 312, 212)
+    pos, rad, q, ctx, b = make(w, emitter_splits=splits, emitter_tile=tile)
+    cfg = celes.celes_launch_config(ctx)
+    assert cfg["emitter_tile"] == tile
+    assert rel(gpu_coupling(ctx, b), orc.coupling_matvec(pos, w.k, w.lmax, b)) <= MATVEC_TOL
+
+
+def test_single_sphere_and_pair():
+    k = workloads.C1.k
+    q = fields.mie_coefficients(3, k, [100.0], workloads.N_SPHERE)
+    ctx = celes.celes_setup(np.zeros((1, 3)), [100.0], q, k, 3)
+    b = workloads.gaussian_coefficients(1, 30, 5)
+    assert np.all(gpu_coupling(ctx, b) == 0)                      # N = 1: W b = 0 (sum over i' != i is empty)
+    out = celes.celes_system_matvec(ctx, torch.from_numpy(b).cuda()).cpu().numpy()
+    assert np.array_equal(out, b)
+    pos = np.array([[0.0, 0, 0], [230.0, 40.0, -60.0]])
+    q2 = fields.mie_coefficients(3, k, [100.0, 100.0], workloads.N_SPHERE)
+    ctx2 = celes.celes_setup(pos, [100.0, 100.0], q2, k, 3)
+    b2 = workloads.gaussian_coefficients(2, 30, 6)
+    assert rel(gpu_coupling(ctx2, b2), orc.coupling_matvec(pos, k, 3, b2)) <= MATVEC_TOL
+
+
+def test_on_axis_and_lattice_pairs():
+    """d parallel to z (rho = 0, reading R8) and axis-aligned lattice pairs."""
+    k = workloads.C1.k
+    g = np.arange(3) * 260.0
+    pos = np.array([[x, y, z] for x in g for y in g for z in g])
+    rad = np.full(len(pos), 100.0)
+    q = fields.mie_coefficients(3, k, rad, workloads.N_SPHERE)
+    ctx = celes.celes_setup(pos, rad, q, k, 3)
+    b = workloads.gaussian_coefficients(len(pos), 30, 7)
+    assert rel(gpu_coupling(ctx, b), orc.coupling_matvec(pos, k, 3, b)) <= MATVEC_TOL
+
+
+def test_far_from_origin_coordinates():
+    """FP64 subtraction of the centres: a cluster 1 mm away from the origin keeps the tolerance."""
+    w = workloads.C1
+    pos, rad = workloads.positions(w)
+    pos = pos + np.array([1.0e6, -7.0e5, 3.0e5])
+    q = fields.mie_coefficients(w.lmax, w.k, rad, workloads.N_SPHERE)
+    ctx = celes.celes_setup(pos, rad, q, w.k, w.lmax)
+    b = workloads.gaussian_coefficients(w.N, w.nmax, w.seed_b)
+    assert rel(gpu_coupling(ctx, b), orc.coupling_matvec(pos, w.k, w.lmax, b)) <= MATVEC_TOL
+
+
+def test_c2_coupling_and_system_matvec_full_oracle():
+    w = workloads.C2
+    pos, rad, q, ctx, b = make(w)
+    ref = orc.coupling_matvec(pos, w.k, w.lmax, b)
+    assert rel(gpu_coupling(ctx, b), ref) <= MATVEC_TOL
+    out = celes.celes_system_matvec(ctx, torch.from_numpy(b).cuda()).cpu().numpy()
+    qo = orc.mie_q(w.lmax, w.k, rad, workloads.N_SPHERE)
+    assert rel(out, b.astype(np.complex128) - orc.t_diagonal(qo, w.lmax) * ref) <= MATVEC_TOL
+
+
+def test_host_buffer_entry_points():
+    w = workloads.C1
+    pos, rad, q, ctx, b = make(w)
+    y = celes.celes_coupling_matvec_host(ctx, b)
+    assert np.array_equal(y, gpu_coupling(ctx, b))
+    out = celes.celes_system_matvec_host(ctx, b)
+    assert np.array_equal(out, celes.celes_system_matvec(ctx, torch.from_numpy(b).cuda()).cpu().numpy())
+
+
+def test_parity_relation_on_gpu_output():
+    """P4 on the GPU path: W^{i'i}_{nn'} = (-1)^{l+l'+tau+tau'} W^{ii'}_{nn'}: probe with unit vectors."""
+    k = workloads.C1.k
+    pos = np.array([[0.0, 0, 0], [-80.0, 250.0, 150.0]])
+    q = fields.mie_coefficients(3, k, [100.0, 100.0], workloads.N_SPHERE)
+    ctx = celes.celes_setup(pos, [100.0, 100.0], q, k, 3)
+    idx = orc.multi_indices(3)
+    for npr in (0, 7, 16, 29):
+        b = np.zeros((2, 30), np.complex64); b[1, npr] = 1          # emitter 1 -> receiver 0: column n' of W^{01}
+        col01 = gpu_coupling(ctx, b)[0]
+        for n in (2, 11, 22):
+            b2 = np.zeros((2, 30), np.complex64); b2[0, npr] = 1    # W^{10}[n, n']
+            w10 = gpu_coupling(ctx, b2)[1][n]
+            sign = (-1) ** (idx[n][1] + idx[npr][1] + idx[n][0] + idx[npr][0])
+            assert abs(w10 - sign * col01[n]) <= 2e-5 * max(1.0, abs(w10))
+
+
+def test_c3_sampled_receivers():
+    w = workloads.C3
+    pos, rad, q, ctx, b = make(w)
+    y = gpu_coupling(ctx, b)
+    recv = workloads.sample_receivers(w.N, 256, 303)
+    ref = orc.coupling_matvec(pos, w.k, w.lmax, b, receivers=recv)
+    assert rel(y[recv], ref) <= MATVEC_TOL
+
+
+@pytest.mark.slow
+def test_c4_sampled_receivers_full_size():
+    """BASELINE.json config 4 at full size in the launch configuration bench.py times; the oracle checks 256
+    seeded receivers (full emitter sum each)."""
+    w = workloads.C4
+    pos, rad, q, ctx, b = make(w)
+    y = gpu_coupling(ctx, b)
+    recv = workloads.sample_receivers(w.N, 256, 304)
+    ref = orc.coupling_matvec(pos, w.k, w.lmax, b, receivers=recv)
+    assert rel(y[recv], ref) <= MATVEC_TOL
+
+
+def test_c2_solve_against_oracle_gmres():
+    w = workloads.scaled(workloads.C2, 300)
+    pos, rad, q, ctx, _ = make(w)
+    qo = orc.mie_q(w.lmax, w.k, rad, workloads.N_SPHERE)
+    a_in = orc.plane_wave_a_in(pos, w.k, w.lmax)
+    xref, oinfo = orc.solve_gmres(pos, w.k, w.lmax, qo, a_in, rtol=1e-10)
+    assert oinfo["rel_residual"] <= 1e-10
+    x = torch.zeros(w.N, w.nmax, dtype=torch.complex64, device="cuda")
+    info = celes.celes_solve(ctx, torch.from_numpy(a_in.astype(np.complex64)).cuda(), x, restart=30, rtol=1e-4)
+    assert info["converged"]
+    assert rel(x.cpu().numpy(), xref) <= SOLVE_TOL
+    # optical theorem on the GPU solution (P8): lossless spheres -> C_ext = C_sca
+    xg = x.cpu().numpy().astype(np.complex128)
+    cext = orc.extinction_cross_section(w.k, a_in, xg)
+    csca = orc.scattering_cross_section(pos, w.k, w.lmax, xg)
+    assert abs(cext - csca) / cext <= 2e-3
+
+
+def test_c5_shaped_solve_sampled_residual():
+    """P12: a-posteriori residual of the GPU solution evaluated by the ORACLE on sampled receivers."""
+    w = workloads.scaled(workloads.C5, 2000)
+    pos, rad, q, ctx, _ = make(w)
+    qo = orc.mie_q(w.lmax, w.k, rad, workloads.N_SPHERE)
+    a_in = orc.plane_wave_a_in(pos, w.k, w.lmax)
+    x = torch.zeros(w.N, w.nmax, dtype=torch.complex64, device="cuda")
+    info = celes.celes_solve(ctx, torch.from_numpy(a_in.astype(np.complex64)).cuda(), x, restart=30, rtol=1e-4)
+    assert info["converged"], info
+    xg = x.cpu().numpy().astype(np.complex128)
+    recv = workloads.sample_receivers(w.N, 128, 305)
+    Wx = orc.coupling_matvec(pos, w.k, w.lmax, xg, receivers=recv)
+    T = orc.t_diagonal(qo, w.lmax)[recv]
+    rhs = T * a_in[recv]
+    res = rhs - (xg[recv] - T * Wx)
+    assert np.linalg.norm(res) / np.linalg.norm(rhs) <= 3e-4

@@ -1,0 +1,154 @@
+"""CPU-only checks of the product's host side: the C-ABI library loads and exports every symbol of
+include/celes.h, argument validation, the run-time translation table against the oracle's a5/b5 and against
+the immediates baked into the generated kernel bodies, and the input-preparation helpers against the oracle."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+import paper_1706_02145_b200 as celes
+from paper_1706_02145_b200 import binding, fields, workloads
+from paper_1706_02145_b200 import build as celes_build
+from oracle import celes_oracle as orc
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _built():
+    celes_build.build()
+
+
+def test_library_exports_every_declared_symbol():
+    hdr = open(os.path.join(ROOT, "include", "celes.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b(celes_[a-z0-9_]+)\s*\(", hdr))
+    assert declared == set(binding.EXPORTS)
+    L = binding.lib()
+    for name in declared:
+        assert hasattr(L, name), name
+
+
+def test_nmax_and_strerror():
+    assert [celes.celes_nmax(l) for l in (1, 2, 3, 4)] == [6, 16, 30, 48]
+    with pytest.raises(celes.CelesError):
+        celes.celes_nmax(0)
+    with pytest.raises(celes.CelesError):
+        celes.celes_nmax(5)
+    for code in (0, -1, -2, -3, -4):
+        assert binding.strerror(code) and "unknown" not in binding.strerror(code)
+    assert "unknown" in binding.strerror(-99)
+
+
+def _setup_rc(N, lmax, pos, rad, q, k, out=True):
+    L = binding.lib()
+    h = ctypes.c_void_p(123)
+    rc = L.celes_setup(ctypes.byref(h) if out else None, N, lmax,
+                       None if pos is None else pos.ctypes.data, None if rad is None else rad.ctypes.data,
+                       None if q is None else q.ctypes.data, k, None, None)
+    return rc, h.value
+
+
+def test_setup_rejects_bad_arguments_before_touching_the_gpu():
+    pos = np.array([[0., 0, 0], [300., 0, 0]]); rad = np.array([100., 100.]); q = np.zeros((2, 2, 3), complex)
+    k = 0.0114
+    assert _setup_rc(2, 3, pos, rad, q, k, out=False)[0] == binding.CELES_EINVAL
+    assert _setup_rc(0, 3, pos, rad, q, k) == (binding.CELES_EINVAL, None)
+    assert _setup_rc(2, 0, pos, rad, q, k)[0] == binding.CELES_EINVAL
+    assert _setup_rc(2, 5, pos, rad, q, k)[0] == binding.CELES_EINVAL
+    assert _setup_rc(2, 3, None, rad, q, k)[0] == binding.CELES_EINVAL
+    assert _setup_rc(2, 3, pos, None, q, k)[0] == binding.CELES_EINVAL
+    assert _setup_rc(2, 3, pos, rad, None, k)[0] == binding.CELES_EINVAL
+    assert _setup_rc(2, 3, pos, rad, q, 0.0)[0] == binding.CELES_EINVAL
+    assert _setup_rc(2, 3, pos, rad, q, float("nan"))[0] == binding.CELES_EINVAL
+    bad = pos.copy(); bad[1, 1] = np.inf
+    assert _setup_rc(2, 3, bad, rad, q, k)[0] == binding.CELES_EINVAL
+    close = pos.copy(); close[1, 0] = 199.0           # overlapping spheres (PAPER.md:33 needs disjoint spheres)
+    assert _setup_rc(2, 3, close, rad, q, k)[0] == binding.CELES_EINVAL
+    badr = rad.copy(); badr[0] = -1.0
+    assert _setup_rc(2, 3, pos, badr, q, k)[0] == binding.CELES_EINVAL
+
+
+def test_overlap_check_finds_a_single_overlap_in_a_large_packing():
+    w = workloads.scaled(workloads.C3, 3000)
+    pos, rad = workloads.positions(w)
+    q = np.zeros((w.N, 2, w.lmax), complex)
+    rc, _ = _setup_rc(w.N, w.lmax, pos, rad, q, w.k)
+    assert rc in (binding.CELES_OK, binding.CELES_ECUDA)       # valid packing: passes validation (no GPU here -> ECUDA)
+    bad = pos.copy(); bad[1717] = bad[42] + np.array([150.0, 0.0, 10.0])
+    assert _setup_rc(w.N, w.lmax, bad, rad, q, w.k)[0] == binding.CELES_EINVAL
+
+
+def test_compute_entry_points_reject_null():
+    L = binding.lib()
+    assert L.celes_coupling_matvec(None, None, None, None) == binding.CELES_EINVAL
+    assert L.celes_system_matvec(None, None, None, None) == binding.CELES_EINVAL
+    assert L.celes_solve(None, None, None, None, None, None) == binding.CELES_EINVAL
+    L.celes_destroy(None)
+
+
+@pytest.mark.parametrize("lmax", [1, 2, 3, 4])
+def test_translation_table_matches_oracle_a5_b5(lmax):
+    """The library's run-time table (own 3j code) against the oracle's Racah-formula a5/b5, with the index swap
+    of eq. (7): W_{(lm),(l'm')} uses a5(l',m'|l,m|p)."""
+    a, b = celes.celes_translation_table(lmax)
+    for l in range(1, lmax + 1):
+        for m in range(-l, l + 1):
+            for lp in range(1, lmax + 1):
+                for mp in range(-lp, lp + 1):
+                    r, c = (l - 1) * (l + 1) + m + l, (lp - 1) * (lp + 1) + mp + lp
+                    for p in range(0, 2 * lmax + 1):
+                        va, vb = orc.a5(lp, mp, l, m, p), orc.b5(lp, mp, l, m, p)
+                        if p < abs(l - lp) or p > l + lp:
+                            assert a[r, c, p] == 0 and b[r, c, p] == 0
+                            continue
+                        assert abs(va.imag) < 1e-13 and abs(vb.real) < 1e-13
+                        assert abs(a[r, c, p] - va.real) < 1e-12
+                        assert abs(b[r, c, p] - vb.imag) < 1e-12
+
+
+@pytest.mark.parametrize("lmax", [1, 2, 3, 4])
+def test_generated_kernel_bodies_carry_the_table_counts(lmax):
+    """The generated straight-line bodies state how many non-zero a5 / b5 terms (p >= |m'-m|) they contain; the
+    same count from the library's table."""
+    a, b = celes.celes_translation_table(lmax)
+    na = nb = 0
+    for l in range(1, lmax + 1):
+        for m in range(-l, l + 1):
+            for lp in range(1, lmax + 1):
+                for mp in range(-lp, lp + 1):
+                    r, c = (l - 1) * (l + 1) + m + l, (lp - 1) * (lp + 1) + mp + lp
+                    for p in range(abs(mp - m), 2 * lmax + 1):
+                        na += abs(a[r, c, p]) > 1e-14
+                        nb += abs(b[r, c, p]) > 1e-14
+    head = open(os.path.join(ROOT, "paper_1706_02145_b200", "csrc", "generated", f"coupling_body_lmax{lmax}.inc")).read(400)
+    mt = re.search(r"a5 (\d+), b5 (\d+)", head)
+    assert (int(mt.group(1)), int(mt.group(2))) == (na, nb)
+
+
+def test_mie_coefficients_match_oracle_B2_B3():
+    k = 2 * np.pi / 550.0
+    R = np.array([100.0, 80.0, 120.0, 95.5])
+    for n in (1.52, 1.52 + 0.1j, 2.4):
+        assert np.abs(fields.mie_coefficients(4, k, R, n) - orc.mie_q(4, k, R, n)).max() < 1e-13
+
+
+def test_plane_wave_coefficients_match_oracle_A13():
+    k = 2 * np.pi / 550.0
+    pos = np.random.default_rng(5).normal(size=(7, 3)) * 400
+    for lmax in (1, 3, 4):
+        a = fields.plane_wave_coefficients(pos, k, lmax)
+        assert np.abs(a - orc.plane_wave_a_in(pos, k, lmax)).max() < 1e-13
+
+
+def test_workloads_are_seeded_and_valid():
+    w = workloads.C1
+    p1, r1 = workloads.positions(w)
+    p2, _ = workloads.positions(w)
+    assert np.array_equal(p1, p2)
+    assert workloads.min_gap(p1, r1) >= workloads.GAP_NM - 1e-9
+    b = workloads.gaussian_coefficients(w.N, w.nmax, w.seed_b)
+    assert b.dtype == np.complex64 and b.shape == (50, 30)
+    assert abs(np.mean(np.abs(b) ** 2) - 1.0) < 0.1

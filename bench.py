@@ -31,9 +31,9 @@ if ROOT not in sys.path:
 
 METRIC = "sphere_pair_translations_per_s"
 UNIT = "pairs/s"
-# Algorithmic FP32 flops per ordered pair of the direct, tau-symmetric translation (DESIGN.md section 6:
-# counted from the generated pair body, FMA = 2): geometry + radial + angular + p-contraction + n'-contraction.
-FLOPS_PER_PAIR = {3: 8.0e3, 4: 21.8e3}
+# FP32 flops per ordered pair of the two pair bodies, counted in the SASS of the coupling kernel's loop body
+# (2 FFMA + FMUL + FADD): geometry + radial functions + rotation/translation + accumulation.
+FLOPS_PER_PAIR = {"rotated": {3: 2324.0, 4: 4844.0}, "direct": {3: 5412.0, 4: 14238.0}}
 FP32_LANES_PER_SM = 128
 
 
@@ -44,6 +44,7 @@ def parse():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--workload", default="C4")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--translation", default="rotated", choices=["rotated", "direct"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=20.0, help="CPU work of the cpu_baseline sample")
     return ap.parse_args()
@@ -186,7 +187,7 @@ def main():
     q = fields.mie_coefficients(w.lmax, w.k, rad, workloads.N_SPHERE)
     b_host = workloads.gaussian_coefficients(w.N, w.nmax, w.seed_b + rank)
     t0 = time.perf_counter()
-    ctx = celes.celes_setup(pos, rad, q, w.k, w.lmax)
+    ctx = celes.celes_setup(pos, rad, q, w.k, w.lmax, translation=args.translation)
     setup_s = time.perf_counter() - t0
     cfg = celes.celes_launch_config(ctx)
     b = torch.from_numpy(b_host).cuda()
@@ -247,7 +248,8 @@ def main():
         sm_mhz = clocks.get("sm_mhz") or peaks.get("sm_max_mhz") or 1965.0
         nominal_peak = 2.0 * FP32_LANES_PER_SM * sm_count * (clocks.get("sm_max_mhz") or 1965.0) * 1e6
         peak_at_clock = 2.0 * FP32_LANES_PER_SM * sm_count * sm_mhz * 1e6
-        flops = FLOPS_PER_PAIR.get(w.lmax, 0.0) * pairs
+        fpp = FLOPS_PER_PAIR[args.translation].get(w.lmax, 0.0)
+        flops = fpp * pairs
         achieved = flops / (ms_per_step * 1e-3)
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -267,7 +269,7 @@ def main():
                          "frac_of_peak_at_observed_clock": achieved / peak_at_clock,
                          "ffma_probe_tflops": {"reg": probe[0] / 1e12, "imm": probe[1] / 1e12, "f32x2": probe[2] / 1e12},
                          "frac_of_ffma_probe": achieved / max(probe.values()),
-                         "flops_per_pair": FLOPS_PER_PAIR.get(w.lmax)},
+                         "flops_per_pair": fpp, "translation": args.translation},
         }
         if not args.no_cpu_baseline and world == 1:
             rate, cores, n_recv, dt = oracle_sample_rate(w, pos, b_host, args.cpu_seconds)

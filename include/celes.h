@@ -46,7 +46,13 @@ typedef struct celes_options {
     int emitter_splits;    /* how many slices the emitter sum of one receiver is cut into (split-K across CTAs);
                               0 = chosen so that the grid fills a whole number of waves on the device */
     int skip_overlap_check;/* 1: do not verify that spheres are disjoint */
+    int translation;       /* how W^{ii'} b^{i'} is evaluated per pair: CELES_TRANSLATION_ROTATED (default) rotates the
+                              emitter coefficients so that d is the z axis, translates along z (diagonal in m) and
+                              rotates back; CELES_TRANSLATION_DIRECT sums (A.6)-(A.8) term by term
+                              (PAPER.md:246-254).  Same result up to FP32 rounding. */
 } celes_options;
+#define CELES_TRANSLATION_ROTATED 0
+#define CELES_TRANSLATION_DIRECT  1
 
 #define CELES_GMRES 0
 typedef struct celes_solve_opts {

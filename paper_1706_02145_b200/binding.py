@@ -18,6 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libceles.so")
 
 CELES_OK, CELES_EINVAL, CELES_ENOMEM, CELES_ECUDA, CELES_ENOCONV = 0, -1, -2, -3, -4
 CELES_GMRES = 0
+CELES_TRANSLATION_ROTATED, CELES_TRANSLATION_DIRECT = 0, 1
 CELES_MAX_HISTORY = 4096
 EXPORTS = ["celes_setup", "celes_coupling_matvec", "celes_system_matvec", "celes_coupling_matvec_host",
            "celes_system_matvec_host", "celes_solve", "celes_destroy", "celes_strerror", "celes_nmax",
@@ -31,7 +32,8 @@ class CelesError(RuntimeError):
 
 
 class celes_options(ctypes.Structure):
-    _fields_ = [("emitter_tile", ctypes.c_int), ("emitter_splits", ctypes.c_int), ("skip_overlap_check", ctypes.c_int)]
+    _fields_ = [("emitter_tile", ctypes.c_int), ("emitter_splits", ctypes.c_int), ("skip_overlap_check", ctypes.c_int),
+                ("translation", ctypes.c_int)]
 
 
 class celes_solve_opts(ctypes.Structure):
@@ -117,7 +119,7 @@ class Context:
 
 
 def celes_setup(pos_xyz, radii, mie_q, k: float, lmax: int, *, emitter_tile: int = 0, emitter_splits: int = 0,
-                skip_overlap_check: bool = False, stream=None) -> Context:
+                skip_overlap_check: bool = False, translation: str = "rotated", stream=None) -> Context:
     """celes_setup of include/celes.h.  pos_xyz [N,3] float64, radii [N] float64, mie_q [N,2,lmax] complex128 (host)."""
     pos = np.ascontiguousarray(pos_xyz, dtype=np.float64)
     rad = np.ascontiguousarray(radii, dtype=np.float64)
@@ -125,7 +127,10 @@ def celes_setup(pos_xyz, radii, mie_q, k: float, lmax: int, *, emitter_tile: int
     N = pos.shape[0] if pos.ndim == 2 else 0
     if pos.ndim != 2 or pos.shape[1] != 3 or rad.shape != (N,) or q.shape != (N, 2, lmax):
         raise ValueError("celes_setup: pos_xyz [N,3], radii [N], mie_q [N,2,lmax] expected")
-    opt = celes_options(int(emitter_tile), int(emitter_splits), int(bool(skip_overlap_check)))
+    if translation not in ("rotated", "direct"):
+        raise ValueError("translation: 'rotated' or 'direct'")
+    opt = celes_options(int(emitter_tile), int(emitter_splits), int(bool(skip_overlap_check)),
+                        CELES_TRANSLATION_DIRECT if translation == "direct" else CELES_TRANSLATION_ROTATED)
     h = ctypes.c_void_p()
     import torch
     s = _stream(stream) if torch.cuda.is_available() else 0

@@ -25,6 +25,7 @@ struct celes_ctx {
     double k = 0.0;
     int device = 0, sm_count = 0;
     int rblocks = 0, splits = 1, chunk = 0, etile = 32;
+    bool rotated = true;         // rotate / axial-translate / rotate body (default) or the direct sum
     size_t coupling_smem = 0;
     double* kpos = nullptr;      // [N][3] FP64, k * r_i
     float2* tdiag = nullptr;     // [N][nmax] T diagonal Q^i_{tau,l} expanded over m (B.1)
@@ -53,49 +54,34 @@ using celes::kBlock;
         }                                             \
     } while (0)
 
-template <int LMAX>
+template <int LMAX, bool ROT>
 int launch_coupling_t(const celes_ctx* c, cudaStream_t s) {
     const size_t smem = celes::coupling_smem_bytes<LMAX>(c->etile);
     dim3 grid(c->rblocks, c->splits);
-    celes::coupling_kernel<LMAX><<<grid, kBlock, smem, s>>>(c->N, c->chunk, c->etile, c->kpos, c->bpm, c->ypart);
+    celes::coupling_kernel<LMAX, ROT><<<grid, kBlock, smem, s>>>(c->N, c->chunk, c->etile, c->kpos, c->bpm, c->ypart);
     return cudaGetLastError() == cudaSuccess ? CELES_OK : CELES_ECUDA;
 }
 
-template <int LMAX>
-int prepare_coupling_t(celes_ctx* c) {
+template <int LMAX, bool ROT>
+int prepare_coupling_t(celes_ctx* c, int* ctas_per_sm) {
     const size_t smem = celes::coupling_smem_bytes<LMAX>(c->etile);
     c->coupling_smem = smem;
-    CU_TRY(cudaFuncSetAttribute(celes::coupling_kernel<LMAX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    CU_TRY(cudaFuncSetAttribute(celes::coupling_kernel<LMAX, ROT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, celes::coupling_kernel<LMAX, ROT>, kBlock, smem));
     return CELES_OK;
 }
 
-template <int LMAX>
-int occupancy_t(const celes_ctx* c, int* ctas_per_sm) {
-    CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, celes::coupling_kernel<LMAX>, kBlock,
-                                                         celes::coupling_smem_bytes<LMAX>(c->etile)));
-    return CELES_OK;
-}
+#define CELES_DISPATCH(fn, ...)                                                                  \
+    switch (c->lmax * 2 + (c->rotated ? 1 : 0)) {                                                \
+        case 2: return fn<1, false>(__VA_ARGS__); case 3: return fn<1, true>(__VA_ARGS__);       \
+        case 4: return fn<2, false>(__VA_ARGS__); case 5: return fn<2, true>(__VA_ARGS__);       \
+        case 6: return fn<3, false>(__VA_ARGS__); case 7: return fn<3, true>(__VA_ARGS__);       \
+        case 8: return fn<4, false>(__VA_ARGS__); case 9: return fn<4, true>(__VA_ARGS__);       \
+    }                                                                                            \
+    return CELES_EINVAL
 
-int launch_coupling(const celes_ctx* c, cudaStream_t s) {
-    switch (c->lmax) {
-        case 1: return launch_coupling_t<1>(c, s);
-        case 2: return launch_coupling_t<2>(c, s);
-        case 3: return launch_coupling_t<3>(c, s);
-        case 4: return launch_coupling_t<4>(c, s);
-    }
-    return CELES_EINVAL;
-}
-
-int prepare_coupling(celes_ctx* c, int* ctas_per_sm) {
-    int rc = CELES_EINVAL;
-    switch (c->lmax) {
-        case 1: rc = prepare_coupling_t<1>(c); if (!rc) rc = occupancy_t<1>(c, ctas_per_sm); break;
-        case 2: rc = prepare_coupling_t<2>(c); if (!rc) rc = occupancy_t<2>(c, ctas_per_sm); break;
-        case 3: rc = prepare_coupling_t<3>(c); if (!rc) rc = occupancy_t<3>(c, ctas_per_sm); break;
-        case 4: rc = prepare_coupling_t<4>(c); if (!rc) rc = occupancy_t<4>(c, ctas_per_sm); break;
-    }
-    return rc;
-}
+int launch_coupling(const celes_ctx* c, cudaStream_t s) { CELES_DISPATCH(launch_coupling_t, c, s); }
+int prepare_coupling(celes_ctx* c, int* ctas_per_sm) { CELES_DISPATCH(prepare_coupling_t, c, ctas_per_sm); }
 
 // y = W b (tdiag == nullptr) or out = b - T (W b): pack -> coupling -> finalize, all on stream s.
 int run_matvec(celes_ctx* c, const float2* b, float2* out, bool system, cudaStream_t s) {
@@ -103,11 +89,13 @@ int run_matvec(celes_ctx* c, const float2* b, float2* out, bool system, cudaStre
     const long long nh = (long long)c->N * H;
     const int tb = 256;
     const unsigned gb = (unsigned)((nh + tb - 1) / tb);
-    celes::pack_kernel<<<gb, tb, 0, s>>>(c->N, H, b, c->bpm);
+    if (c->rotated) celes::pack_kernel<true><<<gb, tb, 0, s>>>(c->N, H, b, c->bpm);
+    else celes::pack_kernel<false><<<gb, tb, 0, s>>>(c->N, H, b, c->bpm);
     if (cudaGetLastError() != cudaSuccess) return CELES_ECUDA;
     int rc = launch_coupling(c, s);
     if (rc) return rc;
-    celes::finalize_kernel<<<gb, tb, 0, s>>>(c->N, H, c->splits, c->ypart, system ? c->tdiag : nullptr, b, out);
+    if (c->rotated) celes::finalize_kernel<true><<<gb, tb, 0, s>>>(c->N, H, c->splits, c->ypart, system ? c->tdiag : nullptr, b, out);
+    else celes::finalize_kernel<false><<<gb, tb, 0, s>>>(c->N, H, c->splits, c->ypart, system ? c->tdiag : nullptr, b, out);
     return cudaGetLastError() == cudaSuccess ? CELES_OK : CELES_ECUDA;
 }
 
@@ -284,6 +272,7 @@ int celes_setup(celes_ctx** out, int N, int lmax, const double* pos_xyz, const d
     const bool skip = opt && opt->skip_overlap_check;
     if (!skip && !spheres_disjoint(N, pos_xyz, radii)) return CELES_EINVAL;
     if (opt && (opt->emitter_tile < 0 || opt->emitter_splits < 0 || opt->emitter_tile > 128)) return CELES_EINVAL;
+    if (opt && opt->translation != CELES_TRANSLATION_ROTATED && opt->translation != CELES_TRANSLATION_DIRECT) return CELES_EINVAL;
 
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); return CELES_ECUDA; }
@@ -298,6 +287,7 @@ int celes_setup(celes_ctx** out, int N, int lmax, const double* pos_xyz, const d
     if (cudaGetDeviceProperties(&prop, c->device) != cudaSuccess) return fail(CELES_ECUDA);
     c->sm_count = prop.multiProcessorCount;
     c->etile = (opt && opt->emitter_tile > 0) ? opt->emitter_tile : 32;
+    c->rotated = !(opt && opt->translation == CELES_TRANSLATION_DIRECT);
     c->rblocks = (N + kBlock - 1) / kBlock;
     int ctas_per_sm = 1;
     rc = prepare_coupling(c, &ctas_per_sm);
@@ -306,18 +296,21 @@ int celes_setup(celes_ctx** out, int N, int lmax, const double* pos_xyz, const d
     if (opt && opt->emitter_splits > 0) {
         c->splits = std::min(opt->emitter_splits, N);
     } else {
-        // Split the emitter sum so that the grid is a whole number of waves (slots = SMs x resident CTAs):
-        // the smallest number of waves that gives every CTA at least ~256 emitters, at most 16 waves.
+        // Split the emitter sum so that the grid is a whole number of waves (slots = SMs x resident CTAs): among
+        // 1..16 waves take the split with the best fill (all CTAs do equal work, so a full last wave means no
+        // tail), slightly preferring more waves, with at least 96 emitters per CTA.
         const long long slots = (long long)c->sm_count * ctas_per_sm;
+        const long long maxsp = std::max<long long>(1, N / 96);
         long long best = 1;
+        double best_score = -1.0;
         for (long long waves = 1; waves <= 16; ++waves) {
-            long long sp = std::max<long long>(1, (waves * slots) / c->rblocks);
-            if (sp * c->rblocks > waves * slots) continue;
-            best = sp;
-            if ((double)sp * c->rblocks >= 0.9 * waves * slots && waves >= 2) break;
+            const long long sp = std::min(maxsp, std::max<long long>(1, (waves * slots) / c->rblocks));
+            const long long used_waves = (sp * c->rblocks + slots - 1) / slots;
+            const double eff = (double)sp * c->rblocks / ((double)used_waves * slots);
+            const double score = eff - 0.02 / (double)used_waves;
+            if (score > best_score + 1e-12) { best_score = score; best = sp; }
         }
-        const long long maxsp = std::max<long long>(1, N / 256);
-        c->splits = (int)std::max<long long>(1, std::min<long long>(best, maxsp));
+        c->splits = (int)best;
     }
     c->chunk = (N + c->splits - 1) / c->splits;
     c->splits = (N + c->chunk - 1) / c->chunk;

@@ -1,6 +1,7 @@
 // coupling_kernel.cuh -- device kernels of y = W b (steps H1-H9 of DESIGN.md section 5).
 //
-//   pack_kernel      b [N][nmax] -> bpm [N][nmax] = [b_1 + b_2 | b_1 - b_2]      (tau-block symmetry of W)
+//   pack_kernel      b [N][nmax] -> bpm [N][nmax]: DIRECT  [b_1 + b_2 | b_1 - b_2]  (tau-block symmetry of W)
+//                                                  ROTATED orthonormal [tau S|A][l][u_0,u+_1,u-_1,..] basis
 //   coupling_kernel  tiled (receiver-block x emitter-block) translation; one thread per receiver, the
 //                    emitter tile (coefficients + FP64 centres) staged through shared memory, FP32 complex
 //                    accumulation in registers (lmax <= 3) or in a conflict-free shared-memory slab (lmax = 4)
@@ -17,15 +18,48 @@ constexpr int kBlock = 128;          // receivers (threads) per CTA
 __host__ __device__ constexpr int nmax_of(int lmax) { return 2 * lmax * (lmax + 2); }
 
 // ---------------------------------------------------------------------------------------------------------
-// b -> [b_+ | b_-].  One thread per (sphere, index inside a tau block).
+// b -> work basis.  One thread per (sphere, index q inside a tau block).
+//   DIRECT : [b_1 + b_2 | b_1 - b_2], index order unchanged.
+//   ROTATED: orthonormal basis of gen_rotated_body.py: x_S/A = (x_1 +- x_2)/sqrt2, then per l
+//            [u_0 = x_0, u+_m = (x_m + x_-m)/sqrt2, u-_m = (x_m - x_-m)/sqrt2, m = 1..l] at q = l^2-1 + {0, 2m-1, 2m}.
+__device__ __forceinline__ void split_q(int q, int& l, int& pos) {
+    l = 1;
+    while ((l + 1) * (l + 1) - 1 <= q) ++l;
+    pos = q - (l * l - 1);
+}
+
+template <bool ROTATED>
 __global__ void pack_kernel(int N, int H, const float2* __restrict__ b, float2* __restrict__ bpm) {
     const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= (long long)N * H) return;
     const long long i = t / H;
     const int q = (int)(t - i * H);
-    const float2 b1 = b[i * 2 * H + q], b2 = b[i * 2 * H + H + q];
-    bpm[i * 2 * H + q] = make_float2(b1.x + b2.x, b1.y + b2.y);
-    bpm[i * 2 * H + H + q] = make_float2(b1.x - b2.x, b1.y - b2.y);
+    const float2* b1 = b + i * 2 * H;
+    const float2* b2 = b1 + H;
+    float2 s, a;
+    if (!ROTATED) {
+        s = make_float2(b1[q].x + b2[q].x, b1[q].y + b2[q].y);
+        a = make_float2(b1[q].x - b2[q].x, b1[q].y - b2[q].y);
+    } else {
+        int l, pos;
+        split_q(q, l, pos);
+        const int c0 = l * l - 1 + l;                       // index of m = 0 inside the tau block
+        if (pos == 0) {
+            const float r = 0.70710678118654752f;
+            s = make_float2(r * (b1[c0].x + b2[c0].x), r * (b1[c0].y + b2[c0].y));
+            a = make_float2(r * (b1[c0].x - b2[c0].x), r * (b1[c0].y - b2[c0].y));
+        } else {
+            const int m = (pos + 1) >> 1;
+            const float sg = (pos & 1) ? 0.5f : -0.5f;      // u+ : x_m + x_-m ; u- : x_m - x_-m ; (1/sqrt2)^2 = 1/2
+            const float2 p1 = b1[c0 + m], n1 = b1[c0 - m], p2 = b2[c0 + m], n2 = b2[c0 - m];
+            const float2 u1 = make_float2(0.5f * p1.x + sg * n1.x, 0.5f * p1.y + sg * n1.y);
+            const float2 u2 = make_float2(0.5f * p2.x + sg * n2.x, 0.5f * p2.y + sg * n2.y);
+            s = make_float2(u1.x + u2.x, u1.y + u2.y);
+            a = make_float2(u1.x - u2.x, u1.y - u2.y);
+        }
+    }
+    bpm[i * 2 * H + q] = s;
+    bpm[i * 2 * H + H + q] = a;
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -73,7 +107,7 @@ constexpr size_t coupling_smem_bytes(int etile) {
 // grid = (ceil(N / kBlock), splits).  CTA (bx, by) translates emitters [by*chunk, min(N, (by+1)*chunk)) to
 // receivers bx*kBlock + tid and writes its partial sums to ypart[by][receiver][q].
 //   kpos  [N][3] FP64: k * r_i.  The subtraction r_i - r_i' is done in FP64, everything after it in FP32.
-template <int LMAX>
+template <int LMAX, bool ROTATED>
 __global__ void __launch_bounds__(kBlock) coupling_kernel(int N, int chunk, int etile,
                                                           const double* __restrict__ kpos,
                                                           const float2* __restrict__ bpm,
@@ -114,7 +148,7 @@ __global__ void __launch_bounds__(kBlock) coupling_kernel(int N, int chunk, int 
             const float dz = (float)(zi - spos[3 * e + 2]);
             const float2* be = sb + e * NMAX;
             auto bload = [be](int q) { return be[q]; };        // same address in every lane: LDS broadcast
-            pair_translate<LMAX>(dx, dy, dz, bload, yacc);
+            pair_translate<LMAX, ROTATED>(dx, dy, dz, bload, yacc);
         }
     }
     if (active) {
@@ -125,8 +159,11 @@ __global__ void __launch_bounds__(kBlock) coupling_kernel(int N, int chunk, int 
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// H8-H9: y_1 = (y_+ + y_-)/2, y_2 = (y_+ - y_-)/2 summed over the splits; if tdiag != nullptr the epilogue of
+// H8-H9: sums the emitter splits and returns to the (tau, l, m) basis; if tdiag != nullptr the epilogue of
 // eq. (9) is fused: out = b - T y with T the diagonal Q^i_{tau,l} expanded to [N][nmax].
+//   DIRECT : y_1 = (y_+ + y_-)/2, y_2 = (y_+ - y_-)/2.
+//   ROTATED: inverse of the orthonormal transform of pack_kernel.  One thread per (sphere, (l,m)).
+template <bool ROTATED>
 __global__ void finalize_kernel(int N, int H, int splits, const float2* __restrict__ ypart,
                                 const float2* __restrict__ tdiag, const float2* __restrict__ b,
                                 float2* __restrict__ out) {
@@ -135,13 +172,44 @@ __global__ void finalize_kernel(int N, int H, int splits, const float2* __restri
     const long long i = t / H;
     const int q = (int)(t - i * H);
     const size_t stride = (size_t)N * 2 * H;
-    float pr = 0.f, pi = 0.f, mr = 0.f, mi = 0.f;
-    for (int s = 0; s < splits; ++s) {
-        const float2 yp = ypart[s * stride + i * 2 * H + q], ym = ypart[s * stride + i * 2 * H + H + q];
-        pr += yp.x; pi += yp.y; mr += ym.x; mi += ym.y;
+    float2 y1, y2;
+    if (!ROTATED) {
+        float pr = 0.f, pi = 0.f, mr = 0.f, mi = 0.f;
+        for (int s = 0; s < splits; ++s) {
+            const float2 yp = ypart[s * stride + i * 2 * H + q], ym = ypart[s * stride + i * 2 * H + H + q];
+            pr += yp.x; pi += yp.y; mr += ym.x; mi += ym.y;
+        }
+        y1 = make_float2(0.5f * (pr + mr), 0.5f * (pi + mi));
+        y2 = make_float2(0.5f * (pr - mr), 0.5f * (pi - mi));
+    } else {
+        int l, pos;
+        split_q(q, l, pos);
+        const int m = pos - l;                               // q = l^2-1 + (m + l)
+        const int base = l * l - 1;
+        const int am = m < 0 ? -m : m;
+        const int qa = base + (am ? 2 * am - 1 : 0);         // u+_|m| (or u_0)
+        const int qb = base + 2 * am;                        // u-_|m| (unused for m = 0)
+        float sar = 0.f, sai = 0.f, sbr = 0.f, sbi = 0.f, aar = 0.f, aai = 0.f, abr = 0.f, abi = 0.f;
+        for (int s = 0; s < splits; ++s) {
+            const float2* y = ypart + s * stride + i * 2 * H;
+            const float2 sa = y[qa], aa = y[H + qa];
+            sar += sa.x; sai += sa.y; aar += aa.x; aai += aa.y;
+            if (am) {
+                const float2 sb = y[qb], ab = y[H + qb];
+                sbr += sb.x; sbi += sb.y; abr += ab.x; abi += ab.y;
+            }
+        }
+        float ysr, ysi, yar, yai;                            // tau blocks S and A at (l, m)
+        if (am == 0) { ysr = sar; ysi = sai; yar = aar; yai = aai; }
+        else {
+            const float r = 0.70710678118654752f, sg = m > 0 ? r : -r;
+            ysr = r * sar + sg * sbr; ysi = r * sai + sg * sbi;
+            yar = r * aar + sg * abr; yai = r * aai + sg * abi;
+        }
+        const float r = 0.70710678118654752f;
+        y1 = make_float2(r * (ysr + yar), r * (ysi + yai));
+        y2 = make_float2(r * (ysr - yar), r * (ysi - yai));
     }
-    float2 y1 = make_float2(0.5f * (pr + mr), 0.5f * (pi + mi));
-    float2 y2 = make_float2(0.5f * (pr - mr), 0.5f * (pi - mi));
     const size_t o1 = i * 2 * H + q, o2 = o1 + H;
     if (tdiag != nullptr) {
         const float2 t1 = tdiag[o1], t2 = tdiag[o2], b1 = b[o1], b2 = b[o2];

@@ -18,10 +18,18 @@ struct PairBody;   // specialised by the generated files
 #include "generated/coupling_body_lmax3.inc"
 #include "generated/coupling_body_lmax4.inc"
 
+template <int LMAX>
+struct PairBodyRot;   // rotate / axial-translate / rotate variant (gen_rotated_body.py)
+
+#include "generated/coupling_rot_lmax1.inc"
+#include "generated/coupling_rot_lmax2.inc"
+#include "generated/coupling_rot_lmax3.inc"
+#include "generated/coupling_rot_lmax4.inc"
+
 // dx, dy, dz: components of k (r_i - r_i') (dimensionless), already rounded to FP32 AFTER the subtraction
 // was done in FP64 (coordinate rounding is the dominant FP32 error otherwise).
 // bload(q): emitter coefficient q of [b_+ | b_-];  yacc(q, re, im): y_pm[q] += (re, im).
-template <int LMAX, class BLoad, class YAcc>
+template <int LMAX, bool ROTATED, class BLoad, class YAcc>
 CELES_DEVICE void pair_translate(float dx, float dy, float dz, const BLoad& bload, YAcc& yacc) {
     constexpr int P = 2 * LMAX + 1;
     // ---- H2 geometry: spherical coordinates of d
@@ -51,5 +59,6 @@ CELES_DEVICE void pair_translate(float dx, float dy, float dz, const BLoad& bloa
         hi[p + 1] = fmaf(f, hi[p], -hi[p - 1]);
     }
     // ---- H4-H7 angular functions, p-contraction, n'-contraction (generated)
-    PairBody<LMAX>::run(hr, hi, ct, st, cph, sph, bload, yacc);
+    if (ROTATED) PairBodyRot<LMAX>::run(hr, hi, ct, st, cph, sph, bload, yacc);
+    else PairBody<LMAX>::run(hr, hi, ct, st, cph, sph, bload, yacc);
 }

@@ -47,10 +47,11 @@ def test_c1_coupling_system_and_solve():
     assert rel(x.cpu().numpy(), orc.solve_dense(pos, w.k, w.lmax, qo, a_in)) <= SOLVE_TOL
 
 
+@pytest.mark.parametrize("translation", ["rotated", "direct"])
 @pytest.mark.parametrize("lmax", [1, 2, 3, 4])
-def test_every_lmax_small_cluster(lmax):
+def test_every_lmax_small_cluster(lmax, translation):
     w = workloads.Workload(f"L{lmax}", 77, lmax, 90.0, 110.0, "cube", 1800.0, 0.0, 111, 311, 211)
-    pos, rad, q, ctx, b = make(w)
+    pos, rad, q, ctx, b = make(w, translation=translation)
     assert rel(gpu_coupling(ctx, b), orc.coupling_matvec(pos, w.k, lmax, b)) <= MATVEC_TOL
 
 
@@ -79,14 +80,15 @@ def test_single_sphere_and_pair():
     assert rel(gpu_coupling(ctx2, b2), orc.coupling_matvec(pos, k, 3, b2)) <= MATVEC_TOL
 
 
-def test_on_axis_and_lattice_pairs():
+@pytest.mark.parametrize("translation", ["rotated", "direct"])
+def test_on_axis_and_lattice_pairs(translation):
     """d parallel to z (rho = 0, reading R8) and axis-aligned lattice pairs."""
     k = workloads.C1.k
     g = np.arange(3) * 260.0
     pos = np.array([[x, y, z] for x in g for y in g for z in g])
     rad = np.full(len(pos), 100.0)
     q = fields.mie_coefficients(3, k, rad, workloads.N_SPHERE)
-    ctx = celes.celes_setup(pos, rad, q, k, 3)
+    ctx = celes.celes_setup(pos, rad, q, k, 3, translation=translation)
     b = workloads.gaussian_coefficients(len(pos), 30, 7)
     assert rel(gpu_coupling(ctx, b), orc.coupling_matvec(pos, k, 3, b)) <= MATVEC_TOL
 
@@ -102,14 +104,23 @@ def test_far_from_origin_coordinates():
     assert rel(gpu_coupling(ctx, b), orc.coupling_matvec(pos, w.k, w.lmax, b)) <= MATVEC_TOL
 
 
-def test_c2_coupling_and_system_matvec_full_oracle():
+@pytest.mark.parametrize("translation", ["rotated", "direct"])
+def test_c2_coupling_and_system_matvec_full_oracle(translation):
     w = workloads.C2
-    pos, rad, q, ctx, b = make(w)
+    pos, rad, q, ctx, b = make(w, translation=translation)
     ref = orc.coupling_matvec(pos, w.k, w.lmax, b)
     assert rel(gpu_coupling(ctx, b), ref) <= MATVEC_TOL
     out = celes.celes_system_matvec(ctx, torch.from_numpy(b).cuda()).cpu().numpy()
     qo = orc.mie_q(w.lmax, w.k, rad, workloads.N_SPHERE)
     assert rel(out, b.astype(np.complex128) - orc.t_diagonal(qo, w.lmax) * ref) <= MATVEC_TOL
+
+
+def test_rotated_and_direct_translation_agree():
+    """Two independent evaluations of the same operator inside the library (PAPER.md:185 vs 246-254)."""
+    w = workloads.scaled(workloads.C3, 1500)
+    pos, rad, q, ctx, b = make(w)
+    _, _, _, ctx_d, _ = make(w, translation="direct")
+    assert rel(gpu_coupling(ctx, b), gpu_coupling(ctx_d, b)) <= 2e-5
 
 
 def test_host_buffer_entry_points():
@@ -138,9 +149,10 @@ def test_parity_relation_on_gpu_output():
             assert abs(w10 - sign * col01[n]) <= 2e-5 * max(1.0, abs(w10))
 
 
-def test_c3_sampled_receivers():
+@pytest.mark.parametrize("translation", ["rotated", "direct"])
+def test_c3_sampled_receivers(translation):
     w = workloads.C3
-    pos, rad, q, ctx, b = make(w)
+    pos, rad, q, ctx, b = make(w, translation=translation)
     y = gpu_coupling(ctx, b)
     recv = workloads.sample_receivers(w.N, 256, 303)
     ref = orc.coupling_matvec(pos, w.k, w.lmax, b, receivers=recv)

@@ -45,6 +45,8 @@ def parse():
     ap.add_argument("--workload", default="C4")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--translation", default="rotated", choices=["rotated", "direct"])
+    ap.add_argument("--solve", action="store_true",
+                    help="time celes_solve (plane wave, GMRES(30), rtol 1e-4) on the workload instead (config 5: --workload C5)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=20.0, help="CPU work of the cpu_baseline sample")
     return ap.parse_args()
@@ -161,12 +163,47 @@ def run_reference(args, w):
         "gpu_launches": 0}))
 
 
+def run_solve(args, w):
+    """BASELINE.json config 5: time to solution and iteration count of celes_solve; one JSON line."""
+    import torch
+    import paper_1706_02145_b200 as celes
+    from paper_1706_02145_b200 import fields, workloads
+    torch.cuda.set_device(0)
+    pos, rad = workloads.positions(w)
+    q = fields.mie_coefficients(w.lmax, w.k, rad, workloads.N_SPHERE)
+    ctx = celes.celes_setup(pos, rad, q, w.k, w.lmax, translation=args.translation)
+    a_in = torch.from_numpy(fields.plane_wave_coefficients(pos, w.k, w.lmax).astype(np.complex64)).cuda()
+    x = torch.zeros(w.N, w.nmax, dtype=torch.complex64, device="cuda")
+    celes.celes_solve(ctx, a_in, x, restart=30, rtol=1e-4, max_iters=3)          # warm-up (allocations, caches)
+    runs = []
+    for _ in range(max(1, args.steps)):
+        x.zero_()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        info = celes.celes_solve(ctx, a_in, x, restart=30, rtol=1e-4, max_iters=2000)
+        torch.cuda.synchronize()
+        runs.append((time.perf_counter() - t0, info))
+    secs = [r[0] for r in runs]
+    info = runs[-1][1]
+    print(json.dumps({
+        "metric": "time_to_solution_s", "value": float(np.median(secs)), "unit": "s", "n_gpus": 1, "steps": len(runs),
+        "warmup": 1, "higher_is_better": False, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"{w.name}: N={w.N} lmax={w.lmax} plane wave +z x-pol, GMRES(30) rtol 1e-4",
+                   "translation": args.translation},
+        "iterations": info["iterations"], "matvecs": info["matvecs"], "converged": info["converged"],
+        "rel_residual": info["rel_residual"], "seconds_all": secs,
+        "ms_per_matvec_incl_krylov": 1e3 * float(np.median(secs)) / max(1, info["matvecs"])}))
+
+
 def main():
     args = parse()
     from paper_1706_02145_b200 import workloads
     w = workloads.CONFIGS[args.workload]
     if args.impl == "reference":
         run_reference(args, w)
+        return
+    if args.solve:
+        run_solve(args, w)
         return
 
     import torch

@@ -33,7 +33,12 @@ METRIC = "sphere_pair_translations_per_s"
 UNIT = "pairs/s"
 # FP32 flops per ordered pair of the two pair bodies, counted in the SASS of the coupling kernel's loop body
 # (2 FFMA + FMUL + FADD): geometry + radial functions + rotation/translation + accumulation.
-FLOPS_PER_PAIR = {"rotated": {3: 2324.0, 4: 4844.0}, "direct": {3: 5412.0, 4: 14238.0}}
+FLOPS_PER_PAIR = {"rotated": {3: 2199.0, 4: 4483.0}, "rotated_scalar": {3: 2324.0, 4: 4844.0},
+                  "direct": {3: 5412.0, 4: 14238.0}}
+# FP32 lane operations per pair (an FFMA2 / FMUL2 / FADD2 is two, an FFMA / FMUL / FADD one): the FMA pipe retires 128 per
+# SM per clock whatever their kind, so lane_ops x pairs / (128 x SMs x clock x time) is the pipe utilisation
+LANE_OPS_PER_PAIR = {"rotated": {3: 1315.0, 4: 2594.0}, "rotated_scalar": {3: 1377.0, 4: 2781.0},
+                     "direct": {3: 3042.0, 4: 7983.0}}
 FP32_LANES_PER_SM = 128
 
 
@@ -44,7 +49,7 @@ def parse():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--workload", default="C4")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--translation", default="rotated", choices=["rotated", "direct"])
+    ap.add_argument("--translation", default="rotated", choices=["rotated", "direct", "rotated_scalar"])
     ap.add_argument("--solve", action="store_true",
                     help="time celes_solve (plane wave, GMRES(30), rtol 1e-4) on the workload instead (config 5: --workload C5)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -306,7 +311,9 @@ def main():
                          "frac_of_peak_at_observed_clock": achieved / peak_at_clock,
                          "ffma_probe_tflops": {"reg": probe[0] / 1e12, "imm": probe[1] / 1e12, "f32x2": probe[2] / 1e12},
                          "frac_of_ffma_probe": achieved / max(probe.values()),
-                         "flops_per_pair": fpp, "translation": args.translation},
+                         "flops_per_pair": fpp, "translation": args.translation,
+                         "fma_pipe_utilisation": LANE_OPS_PER_PAIR[args.translation].get(w.lmax, 0.0) * pairs
+                         / (FP32_LANES_PER_SM * sm_count * sm_mhz * 1e6 * ms_per_step * 1e-3)},
         }
         if not args.no_cpu_baseline and world == 1:
             rate, cores, n_recv, dt = oracle_sample_rate(w, pos, b_host, args.cpu_seconds)

@@ -48,11 +48,14 @@ typedef struct celes_options {
     int skip_overlap_check;/* 1: do not verify that spheres are disjoint */
     int translation;       /* how W^{ii'} b^{i'} is evaluated per pair: CELES_TRANSLATION_ROTATED (default) rotates the
                               emitter coefficients so that d is the z axis, translates along z (diagonal in m) and
-                              rotates back; CELES_TRANSLATION_DIRECT sums (A.6)-(A.8) term by term
-                              (PAPER.md:246-254).  Same result up to FP32 rounding. */
+                              rotates back, in packed FP32 pairs (fma.rn.f32x2);
+                              CELES_TRANSLATION_DIRECT sums (A.6)-(A.8) term by term;
+                              CELES_TRANSLATION_ROTATED_SCALAR is the rotated scheme in scalar FP32 instructions.
+                              Same result up to FP32 rounding. */
 } celes_options;
-#define CELES_TRANSLATION_ROTATED 0
-#define CELES_TRANSLATION_DIRECT  1
+#define CELES_TRANSLATION_ROTATED        0
+#define CELES_TRANSLATION_DIRECT         1
+#define CELES_TRANSLATION_ROTATED_SCALAR 2
 
 #define CELES_GMRES 0
 typedef struct celes_solve_opts {

@@ -18,7 +18,9 @@ LIB_PATH = os.path.join(_HERE, "libceles.so")
 
 CELES_OK, CELES_EINVAL, CELES_ENOMEM, CELES_ECUDA, CELES_ENOCONV = 0, -1, -2, -3, -4
 CELES_GMRES = 0
-CELES_TRANSLATION_ROTATED, CELES_TRANSLATION_DIRECT = 0, 1
+CELES_TRANSLATION_ROTATED, CELES_TRANSLATION_DIRECT, CELES_TRANSLATION_ROTATED_SCALAR = 0, 1, 2
+TRANSLATIONS = {"rotated": CELES_TRANSLATION_ROTATED, "direct": CELES_TRANSLATION_DIRECT,
+                "rotated_scalar": CELES_TRANSLATION_ROTATED_SCALAR}
 CELES_MAX_HISTORY = 4096
 EXPORTS = ["celes_setup", "celes_coupling_matvec", "celes_system_matvec", "celes_coupling_matvec_host",
            "celes_system_matvec_host", "celes_solve", "celes_destroy", "celes_strerror", "celes_nmax",
@@ -127,10 +129,10 @@ def celes_setup(pos_xyz, radii, mie_q, k: float, lmax: int, *, emitter_tile: int
     N = pos.shape[0] if pos.ndim == 2 else 0
     if pos.ndim != 2 or pos.shape[1] != 3 or rad.shape != (N,) or q.shape != (N, 2, lmax):
         raise ValueError("celes_setup: pos_xyz [N,3], radii [N], mie_q [N,2,lmax] expected")
-    if translation not in ("rotated", "direct"):
-        raise ValueError("translation: 'rotated' or 'direct'")
+    if translation not in TRANSLATIONS:
+        raise ValueError("translation: one of " + ", ".join(TRANSLATIONS))
     opt = celes_options(int(emitter_tile), int(emitter_splits), int(bool(skip_overlap_check)),
-                        CELES_TRANSLATION_DIRECT if translation == "direct" else CELES_TRANSLATION_ROTATED)
+                        TRANSLATIONS[translation])
     h = ctypes.c_void_p()
     import torch
     s = _stream(stream) if torch.cuda.is_available() else 0

@@ -25,7 +25,7 @@ struct celes_ctx {
     double k = 0.0;
     int device = 0, sm_count = 0;
     int rblocks = 0, splits = 1, chunk = 0, etile = 32;
-    bool rotated = true;         // rotate / axial-translate / rotate body (default) or the direct sum
+    int variant = celes::kRotated;   // CELES_TRANSLATION_*: packed rotated (default), direct sum, scalar rotated
     size_t coupling_smem = 0;
     double* kpos = nullptr;      // [N][3] FP64, k * r_i
     float2* tdiag = nullptr;     // [N][nmax] T diagonal Q^i_{tau,l} expanded over m (B.1)
@@ -54,7 +54,7 @@ using celes::kBlock;
         }                                             \
     } while (0)
 
-template <int LMAX, bool ROT>
+template <int LMAX, int ROT>
 int launch_coupling_t(const celes_ctx* c, cudaStream_t s) {
     const size_t smem = celes::coupling_smem_bytes<LMAX>(c->etile);
     dim3 grid(c->rblocks, c->splits);
@@ -62,7 +62,7 @@ int launch_coupling_t(const celes_ctx* c, cudaStream_t s) {
     return cudaGetLastError() == cudaSuccess ? CELES_OK : CELES_ECUDA;
 }
 
-template <int LMAX, bool ROT>
+template <int LMAX, int ROT>
 int prepare_coupling_t(celes_ctx* c, int* ctas_per_sm) {
     const size_t smem = celes::coupling_smem_bytes<LMAX>(c->etile);
     c->coupling_smem = smem;
@@ -71,13 +71,13 @@ int prepare_coupling_t(celes_ctx* c, int* ctas_per_sm) {
     return CELES_OK;
 }
 
-#define CELES_DISPATCH(fn, ...)                                                                  \
-    switch (c->lmax * 2 + (c->rotated ? 1 : 0)) {                                                \
-        case 2: return fn<1, false>(__VA_ARGS__); case 3: return fn<1, true>(__VA_ARGS__);       \
-        case 4: return fn<2, false>(__VA_ARGS__); case 5: return fn<2, true>(__VA_ARGS__);       \
-        case 6: return fn<3, false>(__VA_ARGS__); case 7: return fn<3, true>(__VA_ARGS__);       \
-        case 8: return fn<4, false>(__VA_ARGS__); case 9: return fn<4, true>(__VA_ARGS__);       \
-    }                                                                                            \
+#define CELES_DISPATCH(fn, ...)                                                                              \
+    switch (c->lmax * 3 + c->variant) {                                                                      \
+        case 3: return fn<1, 0>(__VA_ARGS__); case 4: return fn<1, 1>(__VA_ARGS__); case 5: return fn<1, 2>(__VA_ARGS__);    \
+        case 6: return fn<2, 0>(__VA_ARGS__); case 7: return fn<2, 1>(__VA_ARGS__); case 8: return fn<2, 2>(__VA_ARGS__);    \
+        case 9: return fn<3, 0>(__VA_ARGS__); case 10: return fn<3, 1>(__VA_ARGS__); case 11: return fn<3, 2>(__VA_ARGS__);  \
+        case 12: return fn<4, 0>(__VA_ARGS__); case 13: return fn<4, 1>(__VA_ARGS__); case 14: return fn<4, 2>(__VA_ARGS__); \
+    }                                                                                                        \
     return CELES_EINVAL
 
 int launch_coupling(const celes_ctx* c, cudaStream_t s) { CELES_DISPATCH(launch_coupling_t, c, s); }
@@ -89,13 +89,16 @@ int run_matvec(celes_ctx* c, const float2* b, float2* out, bool system, cudaStre
     const long long nh = (long long)c->N * H;
     const int tb = 256;
     const unsigned gb = (unsigned)((nh + tb - 1) / tb);
-    if (c->rotated) celes::pack_kernel<true><<<gb, tb, 0, s>>>(c->N, H, b, c->bpm);
-    else celes::pack_kernel<false><<<gb, tb, 0, s>>>(c->N, H, b, c->bpm);
+    if (c->variant == celes::kRotated) celes::pack_kernel<celes::kRotated><<<gb, tb, 0, s>>>(c->N, H, b, c->bpm);
+    else if (c->variant == celes::kDirect) celes::pack_kernel<celes::kDirect><<<gb, tb, 0, s>>>(c->N, H, b, c->bpm);
+    else celes::pack_kernel<celes::kRotatedScalar><<<gb, tb, 0, s>>>(c->N, H, b, c->bpm);
     if (cudaGetLastError() != cudaSuccess) return CELES_ECUDA;
     int rc = launch_coupling(c, s);
     if (rc) return rc;
-    if (c->rotated) celes::finalize_kernel<true><<<gb, tb, 0, s>>>(c->N, H, c->splits, c->ypart, system ? c->tdiag : nullptr, b, out);
-    else celes::finalize_kernel<false><<<gb, tb, 0, s>>>(c->N, H, c->splits, c->ypart, system ? c->tdiag : nullptr, b, out);
+    const float2* td = system ? c->tdiag : nullptr;
+    if (c->variant == celes::kRotated) celes::finalize_kernel<celes::kRotated><<<gb, tb, 0, s>>>(c->N, H, c->splits, c->ypart, td, b, out);
+    else if (c->variant == celes::kDirect) celes::finalize_kernel<celes::kDirect><<<gb, tb, 0, s>>>(c->N, H, c->splits, c->ypart, td, b, out);
+    else celes::finalize_kernel<celes::kRotatedScalar><<<gb, tb, 0, s>>>(c->N, H, c->splits, c->ypart, td, b, out);
     return cudaGetLastError() == cudaSuccess ? CELES_OK : CELES_ECUDA;
 }
 
@@ -272,7 +275,7 @@ int celes_setup(celes_ctx** out, int N, int lmax, const double* pos_xyz, const d
     const bool skip = opt && opt->skip_overlap_check;
     if (!skip && !spheres_disjoint(N, pos_xyz, radii)) return CELES_EINVAL;
     if (opt && (opt->emitter_tile < 0 || opt->emitter_splits < 0 || opt->emitter_tile > 128)) return CELES_EINVAL;
-    if (opt && opt->translation != CELES_TRANSLATION_ROTATED && opt->translation != CELES_TRANSLATION_DIRECT) return CELES_EINVAL;
+    if (opt && (opt->translation < 0 || opt->translation > CELES_TRANSLATION_ROTATED_SCALAR)) return CELES_EINVAL;
 
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); return CELES_ECUDA; }
@@ -287,7 +290,7 @@ int celes_setup(celes_ctx** out, int N, int lmax, const double* pos_xyz, const d
     if (cudaGetDeviceProperties(&prop, c->device) != cudaSuccess) return fail(CELES_ECUDA);
     c->sm_count = prop.multiProcessorCount;
     c->etile = (opt && opt->emitter_tile > 0) ? opt->emitter_tile : 32;
-    c->rotated = !(opt && opt->translation == CELES_TRANSLATION_DIRECT);
+    c->variant = opt ? opt->translation : CELES_TRANSLATION_ROTATED;
     c->rblocks = (N + kBlock - 1) / kBlock;
     int ctas_per_sm = 1;
     rc = prepare_coupling(c, &ctas_per_sm);

@@ -2,6 +2,7 @@
 //
 //   pack_kernel      b [N][nmax] -> bpm [N][nmax]: DIRECT  [b_1 + b_2 | b_1 - b_2]  (tau-block symmetry of W)
 //                                                  ROTATED orthonormal [tau S|A][l][u_0,u+_1,u-_1,..] basis
+//                                                  (packed variant: w_m = i u-_m in place of u-_m)
 //   coupling_kernel  tiled (receiver-block x emitter-block) translation; one thread per receiver, the
 //                    emitter tile (coefficients + FP64 centres) staged through shared memory, FP32 complex
 //                    accumulation in registers (lmax <= 3) or in a conflict-free shared-memory slab (lmax = 4)
@@ -28,8 +29,9 @@ __device__ __forceinline__ void split_q(int q, int& l, int& pos) {
     pos = q - (l * l - 1);
 }
 
-template <bool ROTATED>
+template <int VARIANT>
 __global__ void pack_kernel(int N, int H, const float2* __restrict__ b, float2* __restrict__ bpm) {
+    constexpr bool ROTATED = VARIANT != kDirect;
     const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= (long long)N * H) return;
     const long long i = t / H;
@@ -56,6 +58,10 @@ __global__ void pack_kernel(int N, int H, const float2* __restrict__ b, float2* 
             const float2 u2 = make_float2(0.5f * p2.x + sg * n2.x, 0.5f * p2.y + sg * n2.y);
             s = make_float2(u1.x + u2.x, u1.y + u2.y);
             a = make_float2(u1.x - u2.x, u1.y - u2.y);
+            if (VARIANT == kRotated && !(pos & 1)) {        // packed body: w_m = i u-_m
+                s = make_float2(-s.y, s.x);
+                a = make_float2(-a.y, a.x);
+            }
         }
     }
     bpm[i * 2 * H + q] = s;
@@ -66,13 +72,14 @@ __global__ void pack_kernel(int N, int H, const float2* __restrict__ b, float2* 
 // Accumulator policies for y_pm of one receiver.
 template <int NMAX>
 struct YRegs {                       // registers: every index is a literal after unrolling
-    float re[NMAX], im[NMAX];
+    float2 y[NMAX];
     __device__ __forceinline__ void init(float*, int) {
 #pragma unroll
-        for (int q = 0; q < NMAX; ++q) { re[q] = 0.0f; im[q] = 0.0f; }
+        for (int q = 0; q < NMAX; ++q) y[q] = make_float2(0.0f, 0.0f);
     }
-    __device__ __forceinline__ void operator()(int q, float r, float i) { re[q] += r; im[q] += i; }
-    __device__ __forceinline__ float2 get(int q) const { return make_float2(re[q], im[q]); }
+    __device__ __forceinline__ void operator()(int q, float r, float i) { y[q].x += r; y[q].y += i; }
+    __device__ __forceinline__ float2 get(int q) const { return y[q]; }
+    __device__ __forceinline__ void put(int q, float2 v) { y[q] = v; }
     __host__ __device__ static constexpr size_t smem_bytes() { return 0; }
 };
 
@@ -90,6 +97,7 @@ struct YSmem {                       // shared memory slab [q][thread] (float2):
         base[q * kBlock] = v;
     }
     __device__ __forceinline__ float2 get(int q) const { return base[q * kBlock]; }
+    __device__ __forceinline__ void put(int q, float2 v) { base[q * kBlock] = v; }
     __host__ __device__ static constexpr size_t smem_bytes() { return sizeof(float2) * NMAX * kBlock; }
 };
 
@@ -107,7 +115,7 @@ constexpr size_t coupling_smem_bytes(int etile) {
 // grid = (ceil(N / kBlock), splits).  CTA (bx, by) translates emitters [by*chunk, min(N, (by+1)*chunk)) to
 // receivers bx*kBlock + tid and writes its partial sums to ypart[by][receiver][q].
 //   kpos  [N][3] FP64: k * r_i.  The subtraction r_i - r_i' is done in FP64, everything after it in FP32.
-template <int LMAX, bool ROTATED>
+template <int LMAX, int VARIANT>
 __global__ void __launch_bounds__(kBlock) coupling_kernel(int N, int chunk, int etile,
                                                           const double* __restrict__ kpos,
                                                           const float2* __restrict__ bpm,
@@ -148,7 +156,7 @@ __global__ void __launch_bounds__(kBlock) coupling_kernel(int N, int chunk, int 
             const float dz = (float)(zi - spos[3 * e + 2]);
             const float2* be = sb + e * NMAX;
             auto bload = [be](int q) { return be[q]; };        // same address in every lane: LDS broadcast
-            pair_translate<LMAX, ROTATED>(dx, dy, dz, bload, yacc);
+            pair_translate<LMAX, VARIANT>(dx, dy, dz, bload, yacc);
         }
     }
     if (active) {
@@ -163,10 +171,11 @@ __global__ void __launch_bounds__(kBlock) coupling_kernel(int N, int chunk, int 
 // eq. (9) is fused: out = b - T y with T the diagonal Q^i_{tau,l} expanded to [N][nmax].
 //   DIRECT : y_1 = (y_+ + y_-)/2, y_2 = (y_+ - y_-)/2.
 //   ROTATED: inverse of the orthonormal transform of pack_kernel.  One thread per (sphere, (l,m)).
-template <bool ROTATED>
+template <int VARIANT>
 __global__ void finalize_kernel(int N, int H, int splits, const float2* __restrict__ ypart,
                                 const float2* __restrict__ tdiag, const float2* __restrict__ b,
                                 float2* __restrict__ out) {
+    constexpr bool ROTATED = VARIANT != kDirect;
     const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= (long long)N * H) return;
     const long long i = t / H;
@@ -198,6 +207,11 @@ __global__ void finalize_kernel(int N, int H, int splits, const float2* __restri
                 const float2 sb = y[qb], ab = y[H + qb];
                 sbr += sb.x; sbi += sb.y; abr += ab.x; abi += ab.y;
             }
+        }
+        if (VARIANT == kRotated) {                           // packed body: u-_m = -i w_m
+            float t;
+            t = sbr; sbr = sbi; sbi = -t;
+            t = abr; abr = abi; abi = -t;
         }
         float ysr, ysi, yar, yai;                            // tau blocks S and A at (l, m)
         if (am == 0) { ysr = sar; ysi = sai; yar = aar; yai = aai; }

@@ -26,10 +26,35 @@ struct PairBodyRot;   // rotate / axial-translate / rotate variant (gen_rotated_
 #include "generated/coupling_rot_lmax3.inc"
 #include "generated/coupling_rot_lmax4.inc"
 
+// Packed FP32 pairs (sm_100a: fma.rn.f32x2 / mul.rn.f32x2 / add.rn.f32x2 -> SASS FFMA2 / FMUL2 / FADD2).  A float2
+// holds one complex number (re, im); bc2(a) is the broadcast operand (a, a), which ptxas encodes as a scalar
+// register operand of FFMA2, and negations / swapped halves fold into operand modifiers.
+CELES_DEVICE float2 bc2(float a) { return make_float2(a, a); }
+CELES_DEVICE float2 neg2(float2 a) { return make_float2(-a.x, -a.y); }
+CELES_DEVICE float2 fma2(float2 a, float2 b, float2 c) { return __ffma2_rn(a, b, c); }
+CELES_DEVICE float2 mul2(float2 a, float2 b) { return __fmul2_rn(a, b); }
+CELES_DEVICE float2 add2(float2 a, float2 b) { return __fadd2_rn(a, b); }
+CELES_DEVICE float2 sub2(float2 a, float2 b) { return __fadd2_rn(a, neg2(b)); }
+
+template <int LMAX>
+struct PairBodyPk;    // packed (FFMA2) rotate / axial-translate / rotate variant (gen_packed_body.py)
+
+#include "generated/coupling_pk_lmax1.inc"
+#include "generated/coupling_pk_lmax2.inc"
+#include "generated/coupling_pk_lmax3.inc"
+#include "generated/coupling_pk_lmax4.inc"
+
+// How W^{ii'} b^{i'} is evaluated per pair (celes.h: CELES_TRANSLATION_*)
+namespace celes {
+constexpr int kRotated = 0;         // packed FFMA2 rotate / axial-translate / rotate (default)
+constexpr int kDirect = 1;          // term-by-term sum of (A.6)-(A.8)
+constexpr int kRotatedScalar = 2;   // scalar-FFMA rotate / axial-translate / rotate
+}  // namespace celes
+
 // dx, dy, dz: components of k (r_i - r_i') (dimensionless), already rounded to FP32 AFTER the subtraction
 // was done in FP64 (coordinate rounding is the dominant FP32 error otherwise).
-// bload(q): emitter coefficient q of [b_+ | b_-];  yacc(q, re, im): y_pm[q] += (re, im).
-template <int LMAX, bool ROTATED, class BLoad, class YAcc>
+// bload(q): emitter coefficient q in the variant's work basis;  yacc: accumulator policy of the receiver.
+template <int LMAX, int VARIANT, class BLoad, class YAcc>
 CELES_DEVICE void pair_translate(float dx, float dy, float dz, const BLoad& bload, YAcc& yacc) {
     constexpr int P = 2 * LMAX + 1;
     // ---- H2 geometry: spherical coordinates of d
@@ -47,6 +72,14 @@ CELES_DEVICE void pair_translate(float dx, float dy, float dz, const BLoad& bloa
     // to |h_p| because the Neumann part dominates wherever the Bessel part's recurrence is unstable)
     float sx, cx;
     sincosf(x, &sx, &cx);                            // full-range accurate: kd reaches ~1000 rad
+    if constexpr (VARIANT == celes::kRotated) {             // the same recurrence on packed (Re, Im)
+        float2 h[P];
+        h[0] = mul2(bc2(rinv), make_float2(sx, -cx));
+        h[1] = mul2(bc2(rinv), add2(h[0], make_float2(-cx, -sx)));
+#pragma unroll
+        for (int p = 1; p + 1 < P; ++p) h[p + 1] = fma2(bc2((float)(2 * p + 1) * rinv), h[p], neg2(h[p - 1]));
+        PairBodyPk<LMAX>::run(h, ct, st, cph, sph, bload, yacc);
+    } else {
     float hr[P], hi[P];
     hr[0] = sx * rinv;
     hi[0] = -cx * rinv;
@@ -59,6 +92,7 @@ CELES_DEVICE void pair_translate(float dx, float dy, float dz, const BLoad& bloa
         hi[p + 1] = fmaf(f, hi[p], -hi[p - 1]);
     }
     // ---- H4-H7 angular functions, p-contraction, n'-contraction (generated)
-    if (ROTATED) PairBodyRot<LMAX>::run(hr, hi, ct, st, cph, sph, bload, yacc);
+    if constexpr (VARIANT == celes::kRotatedScalar) PairBodyRot<LMAX>::run(hr, hi, ct, st, cph, sph, bload, yacc);
     else PairBody<LMAX>::run(hr, hi, ct, st, cph, sph, bload, yacc);
+    }
 }

@@ -33,11 +33,11 @@ METRIC = "sphere_pair_translations_per_s"
 UNIT = "pairs/s"
 # FP32 flops per ordered pair of the two pair bodies, counted in the SASS of the coupling kernel's loop body
 # (2 FFMA + FMUL + FADD): geometry + radial functions + rotation/translation + accumulation.
-FLOPS_PER_PAIR = {"rotated": {3: 2199.0, 4: 4483.0}, "rotated_scalar": {3: 2324.0, 4: 4844.0},
+FLOPS_PER_PAIR = {"rotated": {3: 1893.0, 4: 3769.0}, "rotated_scalar": {3: 2324.0, 4: 4844.0},
                   "direct": {3: 5412.0, 4: 14238.0}}
 # FP32 lane operations per pair (an FFMA2 / FMUL2 / FADD2 is two, an FFMA / FMUL / FADD one): the FMA pipe retires 128 per
 # SM per clock whatever their kind, so lane_ops x pairs / (128 x SMs x clock x time) is the pipe utilisation
-LANE_OPS_PER_PAIR = {"rotated": {3: 1315.0, 4: 2594.0}, "rotated_scalar": {3: 1377.0, 4: 2781.0},
+LANE_OPS_PER_PAIR = {"rotated": {3: 1223.0, 4: 2350.0}, "rotated_scalar": {3: 1377.0, 4: 2781.0},
                      "direct": {3: 3042.0, 4: 7983.0}}
 FP32_LANES_PER_SM = 128
 

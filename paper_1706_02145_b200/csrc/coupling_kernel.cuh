@@ -14,7 +14,15 @@
 
 namespace celes {
 
-constexpr int kBlock = 128;          // receivers (threads) per CTA
+#ifndef CELES_KBLOCK
+#define CELES_KBLOCK 128
+#endif
+#ifdef CELES_MAXNREG                   // tuning builds: cap the registers of the coupling kernel directly
+#define CELES_COUPLING_BOUNDS __maxnreg__(CELES_MAXNREG)
+#else
+#define CELES_COUPLING_BOUNDS __launch_bounds__(CELES_KBLOCK)
+#endif
+constexpr int kBlock = CELES_KBLOCK;   // receivers (threads) per CTA
 
 __host__ __device__ constexpr int nmax_of(int lmax) { return 2 * lmax * (lmax + 2); }
 
@@ -116,7 +124,7 @@ constexpr size_t coupling_smem_bytes(int etile) {
 // receivers bx*kBlock + tid and writes its partial sums to ypart[by][receiver][q].
 //   kpos  [N][3] FP64: k * r_i.  The subtraction r_i - r_i' is done in FP64, everything after it in FP32.
 template <int LMAX, int VARIANT>
-__global__ void __launch_bounds__(kBlock) coupling_kernel(int N, int chunk, int etile,
+__global__ void CELES_COUPLING_BOUNDS coupling_kernel(int N, int chunk, int etile,
                                                           const double* __restrict__ kpos,
                                                           const float2* __restrict__ bpm,
                                                           float2* __restrict__ ypart) {

@@ -13,7 +13,8 @@ Formulation: that of gen_rotated_body.py (W(d) = D^H Wz(kd) D, PAPER.md:185 name
 
   * the "minus" components are carried as w_m = i u-_m (pack / finalize kernels convert), which makes the
     z-rotation a REAL plane rotation of (u+_m, w_m):   u~+ = c u+ + s w,  w~ = c w - s u+   (c, s = cos, sin m phi);
-    the axial step becomes  y'+ = A u'+ +- beta w',  y'w = A w' -+ beta u'+  (B = i beta, sign = tau block S / A);
+    the axial step becomes  y'+ = A u'+ +- beta w',  y'w = A w' -+ beta u'+  (B = i beta, sign = tau block S / A),
+    which for m >= 1 is diagonal on g+- = u'+ -+ i w' with eigenvalues A +- i s beta (half the complex products);
   * only the unique rotation entries are evaluated: R+-[j][i] = +- R+-[i][j] (d^l_{m'm} = (-1)^{m-m'} d^l_{mm'}),
     detected numerically here, as polynomials in cos^2(theta) times cos / sin factors;
   * the axial coefficients obey A_{l'l m} = +- A_{ll'm}, beta_{l'l m} = +- beta_{ll'm} (detected numerically):
@@ -164,6 +165,8 @@ def emit(lmax):
                 ax[(name, l, lp, m)] = (s, f"{name}{lp}{l}{m}")
                 continue
             var = f"{name}{l}{lp}{m}"
+            if m >= 1:
+                terms = [(p, 0.5 * cc) for (p, cc) in terms]        # eigenvalues (A +- i beta) / 2 below
             p0, c0 = terms[0]
             if abs(abs(c0) - 1.0) < TOL:
                 e = f"h[{p0}]" if c0 > 0 else f"neg2(h[{p0}])"
@@ -175,6 +178,11 @@ def emit(lmax):
             n_ax_ops += len(terms)
             w(f"    const float2 {var} = {e};")
             ax[(name, l, lp, m)] = (1, var)
+        if m >= 1 and l <= lp:
+            # m >= 1: the (u+, w) 2x2 block [[A, s beta], [-s beta, A]] has eigenvectors (1, +-i), eigenvalues A +- i s beta
+            assert A and B
+            w(f"    const float2 E{l}{lp}{m}a = add2(A{l}{lp}{m}, make_float2(-B{l}{lp}{m}.y, B{l}{lp}{m}.x));")
+            w(f"    const float2 E{l}{lp}{m}b = add2(A{l}{lp}{m}, make_float2(B{l}{lp}{m}.y, -B{l}{lp}{m}.x));")
 
     def cmac(acc, sign, kvar, x, first):
         """(P, Q) (+)= sign * (k.x, k.y) * x: the complex product k x = P + i Q is kept as two packed sums with a
@@ -217,29 +225,36 @@ def emit(lmax):
             for mt in range(1, l + 1):
                 terms = [(*R[("m", l, mt - 1, m - 1)], f"zw{l}_{m}") for m in range(1, l + 1)]
                 w(f"      const float2 uw{l}_{mt} = {rsum(terms)};")
-        # (3) axial translation: y'+ = A u'+ +- beta w',  y'w = A w' -+ beta u'+
+        # (3) axial translation.  m = 0: y'+ = A u'+.  m >= 1: y'+ = A u'+ +- beta w', y'w = A w' -+ beta u'+ is
+        # diagonal on g+- = u'+ -+ i w':  y'+ = L+ g+ + L- g-,  y'w = i (L+ g+ - L- g-),  L+- = (A +- i s beta) / 2
+        for mt in range(1, lmax + 1):
+            for lp in range(mt, lmax + 1):
+                w(f"      const float2 gp{lp}_{mt} = add2(up{lp}_{mt}, make_float2(uw{lp}_{mt}.y, -uw{lp}_{mt}.x));")
+                w(f"      const float2 gm{lp}_{mt} = add2(up{lp}_{mt}, make_float2(-uw{lp}_{mt}.y, uw{lp}_{mt}.x));")
         for l in range(1, lmax + 1):
-            for mt in range(0, l + 1):
-                first_p, first_w = True, True
-                for lp in range(max(1, mt), lmax + 1):
+            first = True
+            for lp in range(1, lmax + 1):
+                sa, va = ax[("A", l, lp, 0)]
+                if sa:
+                    cmac(f"yp{l}_0", sa, va, f"up{lp}_0", first)
+                    first = False
+            assert not first
+            w(f"      const float2 yp{l}_0 = add2(yp{l}_0P, make_float2(-yp{l}_0Q.y, yp{l}_0Q.x));")
+            for mt in range(1, l + 1):
+                first = True
+                for lp in range(mt, lmax + 1):
                     sa, va = ax[("A", l, lp, mt)]
                     sb, vb = ax[("B", l, lp, mt)]
-                    if sa:
-                        cmac(f"yp{l}_{mt}", sa, va, f"up{lp}_{mt}", first_p)
-                        first_p = False
-                        if mt:
-                            cmac(f"yw{l}_{mt}", sa, va, f"uw{lp}_{mt}", first_w)
-                            first_w = False
-                    if sb and mt:
-                        cmac(f"yp{l}_{mt}", sb * tsign, vb, f"uw{lp}_{mt}", first_p)
-                        first_p = False
-                        cmac(f"yw{l}_{mt}", -sb * tsign, vb, f"up{lp}_{mt}", first_w)
-                        first_w = False
-                assert not first_p and (mt == 0 or not first_w)
-                # P + i Q: one FADD2 with the swapped-halves, (-,+) operand form
-                w(f"      const float2 yp{l}_{mt} = add2(yp{l}_{mt}P, make_float2(-yp{l}_{mt}Q.y, yp{l}_{mt}Q.x));")
-                if mt:
-                    w(f"      const float2 yw{l}_{mt} = add2(yw{l}_{mt}P, make_float2(-yw{l}_{mt}Q.y, yw{l}_{mt}Q.x));")
+                    assert sa and sb and va[1:] == vb[1:]
+                    base = "E" + va[1:]
+                    plus, minus = ("a", "b") if sa * sb * tsign > 0 else ("b", "a")
+                    cmac(f"zp{l}_{mt}", sa, base + plus, f"gp{lp}_{mt}", first)
+                    cmac(f"zm{l}_{mt}", sa, base + minus, f"gm{lp}_{mt}", first)
+                    first = False
+                w(f"      const float2 zp{l}_{mt}c = add2(zp{l}_{mt}P, make_float2(-zp{l}_{mt}Q.y, zp{l}_{mt}Q.x));")
+                w(f"      const float2 zm{l}_{mt}c = add2(zm{l}_{mt}P, make_float2(-zm{l}_{mt}Q.y, zm{l}_{mt}Q.x));")
+                w(f"      const float2 yp{l}_{mt} = add2(zp{l}_{mt}c, zm{l}_{mt}c);")
+                w(f"      const float2 yw{l}_{mt} = add2(make_float2(-zp{l}_{mt}c.y, zp{l}_{mt}c.x), make_float2(zm{l}_{mt}c.y, -zm{l}_{mt}c.x));")
         # (4) rotate back (transposes), (5) z-rotate back and accumulate
         for l in range(1, lmax + 1):
             o = ts * H + (l - 1) * (l + 1)

@@ -40,6 +40,9 @@ FLOPS_PER_PAIR = {"rotated": {3: 1893.0, 4: 3769.0}, "rotated_scalar": {3: 2324.
 LANE_OPS_PER_PAIR = {"rotated": {3: 1223.0, 4: 2350.0}, "rotated_scalar": {3: 1377.0, 4: 2781.0},
                      "direct": {3: 3042.0, 4: 7983.0}}
 FP32_LANES_PER_SM = 128
+# dram__bytes_read.sum + dram__bytes_write.sum of one coupling-kernel launch, from the ncu --set full captures
+# summarised under profiles/ (r01c_packed_kernel_c4.md, r01b_rotated_kernel_c4.md)
+NCU_DRAM_BYTES_PER_LAUNCH = {("C4", "rotated"): 132.8e6, ("C4", "rotated_scalar"): 132.0e6}
 
 
 def parse():
@@ -244,7 +247,7 @@ def main():
         torch.cuda.synchronize()
 
     # FP32 peak of this GPU at its clocks of the moment (FFMA-only probe)
-    probe = {v: celes.celes_fp32_peak_probe(v, 2048)["flops_per_s"] for v in (0, 1, 2)}
+    probe = {v: celes.celes_fp32_peak_probe(v, 2048)["flops_per_s"] for v in (0, 1, 2, 3, 4)}
     for _ in range(args.warmup):
         celes.celes_coupling_matvec(ctx, b, y)
     barrier()
@@ -293,6 +296,8 @@ def main():
         fpp = FLOPS_PER_PAIR[args.translation].get(w.lmax, 0.0)
         flops = fpp * pairs
         achieved = flops / (ms_per_step * 1e-3)
+        lane_ops = LANE_OPS_PER_PAIR[args.translation].get(w.lmax, 0.0)
+        lane_rate = lane_ops * pairs / (ms_per_step * 1e-3)           # FP32 lane operations per second
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -306,14 +311,19 @@ def main():
                     "d2h_bytes_per_step": int(b_host.nbytes)},
             "gpu_launches": 3 * args.steps,
             "roofline": {"bound": "alu", "achieved": achieved / 1e12, "peak": nominal_peak / 1e12, "unit": "TFLOP/s",
-                         "frac": achieved / nominal_peak, "traffic": None,
+                         "frac": achieved / nominal_peak,
+                         "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get((w.name, args.translation)),
                          "peak_kind": "derived: 2 x 128 FP32 lanes x SMs x clocks.max.sm (DESIGN.md section 7)",
                          "frac_of_peak_at_observed_clock": achieved / peak_at_clock,
-                         "ffma_probe_tflops": {"reg": probe[0] / 1e12, "imm": probe[1] / 1e12, "f32x2": probe[2] / 1e12},
+                         "ffma_probe_tflops": {"reg": probe[0] / 1e12, "imm": probe[1] / 1e12, "f32x2": probe[2] / 1e12,
+                                               "f32x2_3_register_operands": probe[3] / 1e12,
+                                               "f32x2_shared_multiplicand": probe[4] / 1e12},
                          "frac_of_ffma_probe": achieved / max(probe.values()),
                          "flops_per_pair": fpp, "translation": args.translation,
-                         "fma_pipe_utilisation": LANE_OPS_PER_PAIR[args.translation].get(w.lmax, 0.0) * pairs
-                         / (FP32_LANES_PER_SM * sm_count * sm_mhz * 1e6 * ms_per_step * 1e-3)},
+                         "lane_ops_per_pair": lane_ops,
+                         "fma_pipe_utilisation": lane_rate / (FP32_LANES_PER_SM * sm_count * sm_mhz * 1e6),
+                         "lane_rate_vs_3_operand_probe": lane_rate / (0.5 * probe[3]),
+                         "lane_rate_vs_shared_multiplicand_probe": lane_rate / (0.5 * probe[4])},
         }
         if not args.no_cpu_baseline and world == 1:
             rate, cores, n_recv, dt = oracle_sample_rate(w, pos, b_host, args.cpu_seconds)

@@ -130,7 +130,10 @@ int celes_translation_table(int lmax, double* a5_re, double* b5_im);
 
 /* FP32 peak probe: runs an FFMA-only kernel (independent chains, every SM) and reports the achieved
  * FLOP/s (2 flop per FMA).  variant 0: three-register FFMA; 1: FFMA with an immediate multiplicand;
- * 2: packed fma.rn.f32x2.  Synchronises the stream. */
+ * 2: packed fma.rn.f32x2 (all three with operands that stay in the operand reuse cache); 3: packed fma.rn.f32x2 with
+ * three register operands per instruction and none shared by consecutive instructions; 4: as 3 with the packed
+ * multiplicand shared by eight consecutive instructions.  3 and 4 bracket what a stream shaped like the pair body
+ * (coefficient x packed complex + packed accumulator) can sustain.  Synchronises the stream. */
 int celes_fp32_peak_probe(int variant, int iters, double* flops_per_s, double* milliseconds, void* cuda_stream);
 
 #ifdef __cplusplus

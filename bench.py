@@ -55,6 +55,9 @@ def parse():
     ap.add_argument("--translation", default="rotated", choices=["rotated", "direct", "rotated_scalar"])
     ap.add_argument("--solve", action="store_true",
                     help="time celes_solve (plane wave, GMRES(30), rtol 1e-4) on the workload instead (config 5: --workload C5)")
+    ap.add_argument("--precond-edge", type=float, default=0.0,
+                    help="with --solve: lateral edge (nm) of the cuboids of the block-diagonal preconditioner (0 = none)")
+    ap.add_argument("--method", default="gmres", choices=["gmres", "bicgstab"], help="with --solve")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=20.0, help="CPU work of the cpu_baseline sample")
     return ap.parse_args()
@@ -183,12 +186,18 @@ def run_solve(args, w):
     a_in = torch.from_numpy(fields.plane_wave_coefficients(pos, w.k, w.lmax).astype(np.complex64)).cuda()
     x = torch.zeros(w.N, w.nmax, dtype=torch.complex64, device="cuda")
     celes.celes_solve(ctx, a_in, x, restart=30, rtol=1e-4, max_iters=3)          # warm-up (allocations, caches)
+    pc = None
+    if args.precond_edge > 0:
+        celes.celes_precond_setup(ctx, [args.precond_edge, args.precond_edge, 0.0])   # warm-up (cuSOLVER handle, kernels)
     runs = []
     for _ in range(max(1, args.steps)):
         x.zero_()
         torch.cuda.synchronize()
         t0 = time.perf_counter()
-        info = celes.celes_solve(ctx, a_in, x, restart=30, rtol=1e-4, max_iters=2000)
+        if args.precond_edge > 0:                                                # set-up is part of the time to solution
+            pc = celes.celes_precond_setup(ctx, [args.precond_edge, args.precond_edge, 0.0])
+        info = celes.celes_solve(ctx, a_in, x, restart=30, rtol=1e-4, max_iters=2000, precond=pc is not None,
+                                 method=args.method)
         torch.cuda.synchronize()
         runs.append((time.perf_counter() - t0, info))
     secs = [r[0] for r in runs]
@@ -197,7 +206,8 @@ def run_solve(args, w):
         "metric": "time_to_solution_s", "value": float(np.median(secs)), "unit": "s", "n_gpus": 1, "steps": len(runs),
         "warmup": 1, "higher_is_better": False, "dtype": "f32", "data": "synthetic",
         "config": {"workload": f"{w.name}: N={w.N} lmax={w.lmax} plane wave +z x-pol, GMRES(30) rtol 1e-4",
-                   "translation": args.translation},
+                   "translation": args.translation, "method": args.method,
+                   "preconditioner": None if pc is None else dict(pc, edge_nm=args.precond_edge)},
         "iterations": info["iterations"], "matvecs": info["matvecs"], "converged": info["converged"],
         "rel_residual": info["rel_residual"], "seconds_all": secs,
         "ms_per_matvec_incl_krylov": 1e3 * float(np.median(secs)) / max(1, info["matvecs"])}))

@@ -57,16 +57,29 @@ typedef struct celes_options {
 #define CELES_TRANSLATION_DIRECT         1
 #define CELES_TRANSLATION_ROTATED_SCALAR 2
 
-#define CELES_GMRES 0
+#define CELES_GMRES    0
+#define CELES_BICGSTAB 1
+#define CELES_PRECOND_NONE      0
+#define CELES_PRECOND_BLOCKDIAG 1
 typedef struct celes_solve_opts {
-    int method;            /* CELES_GMRES */
+    int method;            /* CELES_GMRES or CELES_BICGSTAB, the paper's two solvers */
     int restart;           /* GMRES restart length; default 30 */
     double rtol;           /* stop when ||T a_in - M x||_2 / ||T a_in||_2 <= rtol; default 1e-4 */
     int max_iters;         /* bound on inner iterations (= system matvecs inside cycles); default 1000 */
+    int precond;           /* CELES_PRECOND_NONE (default) or CELES_PRECOND_BLOCKDIAG: right preconditioning with the
+                              block-diagonal operator of celes_precond_setup; the stopping
+                              criterion stays the TRUE residual of the unpreconditioned system */
 } celes_solve_opts;
 
+typedef struct celes_precond_info {
+    int n_groups;             /* number of non-empty cuboids N_G */
+    int max_group_spheres;    /* largest N_j */
+    long long block_bytes;    /* device memory of the stored blocks, 8 * sum_j (N_j nmax)^2 */
+    double seconds;           /* wall-clock time of celes_precond_setup */
+} celes_precond_info;
+
 typedef struct celes_solve_info {
-    int iterations;        /* inner GMRES iterations performed */
+    int iterations;        /* inner GMRES iterations / BiCGSTAB iterations (two system matvecs each) performed */
     int matvecs;           /* system matvecs, including the true-residual evaluations at restarts */
     int converged;         /* 1 if the TRUE relative residual met rtol */
     double rel_residual;   /* true relative residual ||T a_in - M x|| / ||T a_in|| of the returned x */
@@ -107,6 +120,24 @@ int celes_system_matvec_host(celes_ctx* ctx, const void* b_host, void* out_host,
  * Returns CELES_OK, or CELES_ENOCONV with x and info still filled. */
 int celes_solve(celes_ctx* ctx, const void* a_in_dev, void* x_dev, const celes_solve_opts* o,
                 celes_solve_info* info, void* cuda_stream);
+
+/* Block-diagonal preconditioner (Fig. 1).  The spheres are divided into subsets G_j by an array
+ * of cuboids with edge lengths edge_xyz[3] (unit U; an edge <= 0 means "do not cut along that axis") anchored at the
+ * minimum corner of the centres' bounding box; for every subset the dense block M_j = (1 - T W) restricted to G_j
+ * is assembled on the device, LU-factorised with partial pivoting and inverted; the context stores the inverses
+ * (8 * sum_j (N_j nmax)^2 bytes).  Replaces an earlier preconditioner of the context.  Synchronises.
+ * CELES_EINVAL: bad argument or a subset with more than 25600 / nmax spheres; CELES_ENOMEM: blocks do not fit;
+ * CELES_ECUDA: CUDA / cuSOLVER failure or a singular block. */
+int celes_precond_setup(celes_ctx* ctx, const double* edge_xyz, celes_precond_info* info, void* cuda_stream);
+
+/* z = blockdiag(M_j^{-1}) v (step 4 of PAPER.md:114).  v_dev, z_dev: device, N*nmax complex64, must not alias.
+ * Asynchronous on cuda_stream.  CELES_EINVAL if celes_precond_setup has not succeeded on this context. */
+int celes_precond_apply(celes_ctx* ctx, const void* v_dev, void* z_dev, void* cuda_stream);
+
+/* Host-only (needs no GPU): the cuboid partition celes_precond_setup uses.  pos_xyz host [N][3], edge_xyz host [3];
+ * group_of[i] (host, [N]) receives the subset of sphere i, subsets numbered in lexicographic (cx, cy, cz) order of
+ * the non-empty cuboids; *n_groups (nullable) their number. */
+int celes_partition(int N, const double* pos_xyz, const double* edge_xyz, int* group_of, int* n_groups);
 
 /* Release the context and every device table it owns.  NULL is allowed. */
 void celes_destroy(celes_ctx* ctx);

@@ -314,6 +314,37 @@ def solve_dense(pos, k, lmax, q, a_in) -> np.ndarray:
     return np.linalg.solve(M, rhs(q, lmax, a_in).reshape(N * n)).reshape(N, n)
 
 
+# ----------------------------------------------------------------------------- block-diagonal preconditioner
+def cuboid_partition(pos, edge_xyz):
+    """Step 1 of PAPER.md:111: divide the volume occupied by the spheres into an array of cuboids (edge lengths
+    edge_xyz, anchored at the minimum corner of the centres; an edge <= 0 means no cut along that axis).  Returns a
+    list of index arrays, one per non-empty cuboid, cuboids in lexicographic (cx, cy, cz) order, spheres in
+    index order inside a cuboid."""
+    pos = np.asarray(pos, dtype=np.float64)
+    e = np.broadcast_to(np.asarray(edge_xyz, dtype=np.float64), (3,))
+    cells = np.zeros(pos.shape, dtype=np.int64)
+    for a in range(3):
+        if e[a] > 0:
+            cells[:, a] = np.floor((pos[:, a] - pos[:, a].min()) / e[a]).astype(np.int64)
+    groups = {}
+    for i in range(pos.shape[0]):
+        groups.setdefault(tuple(cells[i]), []).append(i)
+    return [np.array(groups[key], dtype=np.int64) for key in sorted(groups)]
+
+
+def precond_apply(pos, k, lmax, q, edge_xyz, v) -> np.ndarray:
+    """Steps 2-4 of PAPER.md:112-114: z = blockdiag(M_j^{-1}) v with M_j = M restricted to the spheres of G_j,
+    each block solved by dense LU (numpy.linalg.solve)."""
+    pos = np.asarray(pos, dtype=np.float64)
+    N, n = pos.shape[0], nmax_of(lmax)
+    v = np.asarray(v, dtype=np.complex128).reshape(N, n)
+    z = np.zeros_like(v)
+    for idx in cuboid_partition(pos, edge_xyz):
+        Mj = dense_system_matrix(pos[idx], k, lmax, np.asarray(q)[idx])
+        z[idx] = np.linalg.solve(Mj, v[idx].reshape(-1)).reshape(len(idx), n)
+    return z
+
+
 def solve_gmres(pos, k, lmax, q, a_in, rtol=1e-10, restart=200, max_matvecs=2000, x0=None):
     """b solving eq. (8) by restarted GMRES (Saad & Schultz; ref. [26] of the paper) in FP64 with modified
     Gram-Schmidt; the small least-squares problem is solved with numpy.linalg.lstsq at every step (plain, not

@@ -17,14 +17,16 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libceles.so")
 
 CELES_OK, CELES_EINVAL, CELES_ENOMEM, CELES_ECUDA, CELES_ENOCONV = 0, -1, -2, -3, -4
-CELES_GMRES = 0
+CELES_GMRES, CELES_BICGSTAB = 0, 1
+CELES_PRECOND_NONE, CELES_PRECOND_BLOCKDIAG = 0, 1
 CELES_TRANSLATION_ROTATED, CELES_TRANSLATION_DIRECT, CELES_TRANSLATION_ROTATED_SCALAR = 0, 1, 2
 TRANSLATIONS = {"rotated": CELES_TRANSLATION_ROTATED, "direct": CELES_TRANSLATION_DIRECT,
                 "rotated_scalar": CELES_TRANSLATION_ROTATED_SCALAR}
 CELES_MAX_HISTORY = 4096
 EXPORTS = ["celes_setup", "celes_coupling_matvec", "celes_system_matvec", "celes_coupling_matvec_host",
            "celes_system_matvec_host", "celes_solve", "celes_destroy", "celes_strerror", "celes_nmax",
-           "celes_launch_config", "celes_translation_table", "celes_fp32_peak_probe"]
+           "celes_launch_config", "celes_translation_table", "celes_fp32_peak_probe", "celes_precond_setup",
+           "celes_precond_apply", "celes_partition"]
 
 
 class CelesError(RuntimeError):
@@ -40,7 +42,12 @@ class celes_options(ctypes.Structure):
 
 class celes_solve_opts(ctypes.Structure):
     _fields_ = [("method", ctypes.c_int), ("restart", ctypes.c_int), ("rtol", ctypes.c_double),
-                ("max_iters", ctypes.c_int)]
+                ("max_iters", ctypes.c_int), ("precond", ctypes.c_int)]
+
+
+class celes_precond_info(ctypes.Structure):
+    _fields_ = [("n_groups", ctypes.c_int), ("max_group_spheres", ctypes.c_int), ("block_bytes", ctypes.c_longlong),
+                ("seconds", ctypes.c_double)]
 
 
 class celes_solve_info(ctypes.Structure):
@@ -79,6 +86,12 @@ def lib() -> ctypes.CDLL:
         L.celes_launch_config.argtypes = [p] + [ctypes.POINTER(i)] * 4
         L.celes_translation_table.restype = i
         L.celes_translation_table.argtypes = [i, p, p]
+        L.celes_precond_setup.restype = i
+        L.celes_precond_setup.argtypes = [p, p, ctypes.POINTER(celes_precond_info), p]
+        L.celes_precond_apply.restype = i
+        L.celes_precond_apply.argtypes = [p, p, p, p]
+        L.celes_partition.restype = i
+        L.celes_partition.argtypes = [i, p, p, p, ctypes.POINTER(i)]
         L.celes_fp32_peak_probe.restype = i
         L.celes_fp32_peak_probe.argtypes = [i, i, ctypes.POINTER(d), ctypes.POINTER(d), p]
         _LIB = L
@@ -203,12 +216,54 @@ def celes_system_matvec_host(ctx: Context, b_host: np.ndarray, out_host: np.ndar
     return out_host
 
 
-def celes_solve(ctx: Context, a_in, x, *, restart: int = 30, rtol: float = 1e-4, max_iters: int = 1000, stream=None):
-    """Solve eq. (8) in place in x (in: x0, out: b).  Returns a dict with the celes_solve_info fields; raises
-    CelesError on failure other than CELES_ENOCONV (reported as converged = 0)."""
+def celes_precond_setup(ctx: Context, edge_xyz, stream=None) -> dict:
+    """celes_precond_setup of include/celes.h: block-diagonal preconditioner on cuboids of edge lengths edge_xyz
+    (a scalar means a cube).  Returns the celes_precond_info fields."""
+    e = np.ascontiguousarray(np.broadcast_to(np.asarray(edge_xyz, dtype=np.float64), (3,)))
+    info = celes_precond_info()
+    rc = lib().celes_precond_setup(ctx.handle, e.ctypes.data, ctypes.byref(info), _stream(stream))
+    if rc != CELES_OK:
+        raise CelesError(rc, "celes_precond_setup")
+    return {"n_groups": info.n_groups, "max_group_spheres": info.max_group_spheres, "block_bytes": info.block_bytes,
+            "seconds": info.seconds}
+
+
+def celes_precond_apply(ctx: Context, v, z=None, stream=None):
+    """z = blockdiag(M_j^{-1}) v on device tensors."""
+    import torch
+    _check_vec(v, ctx, "v")
+    if z is None:
+        z = torch.empty_like(v)
+    _check_vec(z, ctx, "z")
+    rc = lib().celes_precond_apply(ctx.handle, v.data_ptr(), z.data_ptr(), _stream(stream))
+    if rc != CELES_OK:
+        raise CelesError(rc, "celes_precond_apply")
+    return z
+
+
+def celes_partition(pos_xyz, edge_xyz):
+    """(group_of [N] int32, n_groups): the cuboid partition of celes_precond_setup (host only, needs no GPU)."""
+    pos = np.ascontiguousarray(pos_xyz, dtype=np.float64)
+    e = np.ascontiguousarray(np.broadcast_to(np.asarray(edge_xyz, dtype=np.float64), (3,)))
+    g = np.empty(pos.shape[0], dtype=np.int32)
+    n = ctypes.c_int()
+    rc = lib().celes_partition(pos.shape[0], pos.ctypes.data, e.ctypes.data, g.ctypes.data, ctypes.byref(n))
+    if rc != CELES_OK:
+        raise CelesError(rc, "celes_partition")
+    return g, n.value
+
+
+def celes_solve(ctx: Context, a_in, x, *, restart: int = 30, rtol: float = 1e-4, max_iters: int = 1000,
+                precond: bool = False, method: str = "gmres", stream=None):
+    """Solve eq. (8) in place in x (in: x0, out: b).  precond=True uses the block-diagonal preconditioner built by
+    celes_precond_setup.  Returns a dict with the celes_solve_info fields; raises CelesError on failure other than
+    CELES_ENOCONV (reported as converged = 0)."""
     _check_vec(a_in, ctx, "a_in")
     _check_vec(x, ctx, "x")
-    o = celes_solve_opts(CELES_GMRES, int(restart), float(rtol), int(max_iters))
+    if method not in ("gmres", "bicgstab"):
+        raise ValueError("method: 'gmres' or 'bicgstab'")
+    o = celes_solve_opts(CELES_BICGSTAB if method == "bicgstab" else CELES_GMRES, int(restart), float(rtol), int(max_iters),
+                         CELES_PRECOND_BLOCKDIAG if precond else CELES_PRECOND_NONE)
     info = celes_solve_info()
     rc = lib().celes_solve(ctx.handle, a_in.data_ptr(), x.data_ptr(), ctypes.byref(o), ctypes.byref(info), _stream(stream))
     if rc not in (CELES_OK, CELES_ENOCONV):

@@ -16,6 +16,8 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libceles.so")
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-shared", "-Xcompiler", "-fPIC"]
+# cuSOLVER (LU of the preconditioner blocks); the CUDA toolkit's copy, found at run time through the rpath
+NVCC_LIBS = ["-lcusolver", "-Xlinker", "-rpath=/usr/local/cuda/lib64"]
 
 
 def sources() -> list[str]:
@@ -37,7 +39,7 @@ def build(force: bool = False, regen: bool = False, verbose: bool = False) -> st
         subprocess.run([sys.executable, os.path.join(CSRC, "gen_coupling_body.py")], check=True)
     if force or stale():
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-        cmd = [nvcc, *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []), "-o", LIB, os.path.join(CSRC, "celes.cu")]
+        cmd = [nvcc, *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []), "-o", LIB, os.path.join(CSRC, "celes.cu"), *NVCC_LIBS]
         subprocess.run(cmd, check=True)
     return LIB
 

@@ -12,13 +12,18 @@
 #include <complex>
 #include <cstdint>
 #include <cstring>
+#include <functional>
 #include <new>
 #include <vector>
 
 #include "../../include/celes.h"
 #include "coupling_kernel.cuh"
 #include "krylov_kernels.cuh"
+#include "partition.h"
+#include "precond_kernels.cuh"
 #include "translation_table.h"
+
+#include <cusolverDn.h>
 
 struct celes_ctx {
     int N = 0, lmax = 0, nmax = 0;
@@ -27,6 +32,7 @@ struct celes_ctx {
     int rblocks = 0, splits = 1, chunk = 0, etile = 32;
     int variant = celes::kRotated;   // CELES_TRANSLATION_*: packed rotated (default), direct sum, scalar rotated
     size_t coupling_smem = 0;
+    std::vector<double> pos;     // host copy of the centres [N][3] (partition of the preconditioner)
     double* kpos = nullptr;      // [N][3] FP64, k * r_i
     float2* tdiag = nullptr;     // [N][nmax] T diagonal Q^i_{tau,l} expanded over m (B.1)
     float2* bpm = nullptr;       // [N][nmax] work: [b_+ | b_-]
@@ -40,6 +46,17 @@ struct celes_ctx {
     double2* coef = nullptr;     // [restart+2]
     double2* hsum = nullptr;     // [restart+2]
     double2* hhost = nullptr;    // pinned [restart+2]
+    // block-diagonal preconditioner (celes_precond_setup)
+    bool pc_ready = false;
+    int pc_groups = 0, pc_max_n = 0, pc_ctas = 0;
+    long long pc_elems = 0;      // sum_j n_j^2
+    int* pc_order = nullptr;     // [N]
+    int* pc_grp_offset = nullptr;        // [groups+1]
+    long long* pc_blk_offset = nullptr;  // [groups]
+    int* pc_cta_group = nullptr;         // [pc_ctas]
+    int* pc_cta_row0 = nullptr;          // [pc_ctas]
+    float2* pc_blocks = nullptr;         // explicit inverses M_j^{-1}, column-major, back to back
+    float2* pc_tmp = nullptr;            // [n] work vector of the preconditioned solve
 };
 
 namespace {
@@ -144,12 +161,28 @@ bool spheres_disjoint(int N, const double* pos, const double* rad) {
     return true;
 }
 
+void free_precond(celes_ctx* c) {
+    cudaFree(c->pc_order); cudaFree(c->pc_grp_offset); cudaFree(c->pc_blk_offset); cudaFree(c->pc_cta_group);
+    cudaFree(c->pc_cta_row0); cudaFree(c->pc_blocks); cudaFree(c->pc_tmp);
+    c->pc_order = c->pc_grp_offset = c->pc_cta_group = c->pc_cta_row0 = nullptr;
+    c->pc_blk_offset = nullptr; c->pc_blocks = c->pc_tmp = nullptr;
+    c->pc_ready = false; c->pc_groups = c->pc_max_n = c->pc_ctas = 0; c->pc_elems = 0;
+}
+
 void free_ctx(celes_ctx* c) {
     if (!c) return;
+    free_precond(c);
     cudaFree(c->kpos); cudaFree(c->tdiag); cudaFree(c->bpm); cudaFree(c->ypart);
     cudaFree(c->V); cudaFree(c->rhs); cudaFree(c->tmp); cudaFree(c->partial); cudaFree(c->coef); cudaFree(c->hsum);
     if (c->hhost) cudaFreeHost(c->hhost);
     delete c;
+}
+
+// z = blockdiag(M_j^{-1}) v  (step 4)
+int precond_apply(celes_ctx* c, const float2* v, float2* z, cudaStream_t s) {
+    celes::block_gemv_kernel<<<c->pc_ctas, celes::kGemvRows, (size_t)c->pc_max_n * sizeof(float2), s>>>(
+        c->nmax, c->pc_cta_group, c->pc_cta_row0, c->pc_grp_offset, c->pc_order, c->pc_blk_offset, c->pc_blocks, v, z);
+    return cudaGetLastError() == cudaSuccess ? CELES_OK : CELES_ECUDA;
 }
 
 int ensure_krylov(celes_ctx* c, int restart) {
@@ -360,6 +393,7 @@ int celes_setup(celes_ctx** out, int N, int lmax, const double* pos_xyz, const d
     c->splits = (N + c->chunk - 1) / c->chunk;
 
     const size_t n = (size_t)N * nmax;
+    c->pos.assign(pos_xyz, pos_xyz + 3 * (size_t)N);
     std::vector<double> kp(3 * (size_t)N);
     for (size_t t = 0; t < kp.size(); ++t) kp[t] = k * pos_xyz[t];
     std::vector<float2> td(n);
@@ -432,6 +466,99 @@ int celes_launch_config(const celes_ctx* ctx, int* receiver_blocks, int* emitter
     return CELES_OK;
 }
 
+}  // extern "C"
+
+namespace {
+// BiCGSTAB (van der Vorst; the paper's second solver) on M x = T a_in, optionally right-preconditioned
+// with the block-diagonal operator.  Three small device->host copies per iteration (the inner products that define
+// alpha, omega and rho); every vector operation is a device kernel.  The recursive residual only proposes
+// convergence: the TRUE residual rhs - M x is recomputed then and decides (as in the GMRES path, reading R14);
+// if it disagrees, or on a breakdown (rho = 0, <r^,v> = 0, <t,t> = 0), the iteration restarts from the true residual.
+int solve_bicgstab(celes_ctx* ctx, float2* x, bool pc, double rtol, int max_iters, double fnorm, cudaStream_t s,
+                   int& iterations, int& matvecs, int& converged, double& rel, const std::function<void(double)>& push_hist) {
+    typedef std::complex<double> cd;
+    const long long n = (long long)ctx->N * ctx->nmax;
+    const int eb = (int)std::min<long long>((n + 255) / 256, (long long)ctx->sm_count * 8);
+    float2* V = ctx->V;
+    float2 *rhat = V, *r = V + n, *p = V + 2 * n, *v = V + 3 * n, *sv = V + 4 * n, *t = V + 5 * n, *phat = V + 6 * n,
+           *shat = V + 7 * n;
+    auto d2 = [](cd z) { return make_double2(z.real(), z.imag()); };
+    auto fetch = [&](int k, cd* out) -> int {          // hsum[0..k) -> host
+        CU_TRY(cudaMemcpyAsync(ctx->hhost, ctx->hsum, sizeof(double2) * k, cudaMemcpyDeviceToHost, s));
+        CU_TRY(cudaStreamSynchronize(s));
+        for (int q = 0; q < k; ++q) out[q] = cd(ctx->hhost[q].x, ctx->hhost[q].y);
+        return CELES_OK;
+    };
+    int rc = CELES_OK, restarts = 0;
+    while (true) {
+        rc = run_matvec(ctx, x, ctx->tmp, true, s);                         // true residual
+        if (rc) return rc;
+        ++matvecs;
+        celes::sub_kernel<<<eb, 256, 0, s>>>(n, ctx->rhs, ctx->tmp, r);
+        double beta0 = 0.0;
+        rc = device_norm(ctx, n, r, &beta0, s);
+        if (rc) return rc;
+        rel = beta0 / fnorm;
+        push_hist(rel);
+        if (rel <= rtol) { converged = 1; return CELES_OK; }
+        if (iterations >= max_iters || ++restarts > 50) return CELES_ENOCONV;
+        if (!std::isfinite(rel)) return CELES_ECUDA;
+        CU_TRY(cudaMemcpyAsync(rhat, r, sizeof(float2) * n, cudaMemcpyDeviceToDevice, s));
+        CU_TRY(cudaMemsetAsync(p, 0, sizeof(float2) * n, s));
+        CU_TRY(cudaMemsetAsync(v, 0, sizeof(float2) * n, s));
+        cd rho = 1.0, alpha = 1.0, omega = 1.0, rho_new = cd(beta0 * beta0, 0.0);
+        bool first = true;
+        while (iterations < max_iters) {
+            const cd beta = first ? cd(0.0) : (rho_new / rho) * (alpha / omega);
+            // p = r + beta (p - omega v)
+            celes::lincomb_kernel<<<eb, 256, 0, s>>>(n, d2(1.0), r, d2(beta), p, d2(-beta * omega), v, p);
+            first = false;
+            const float2* pin = p;
+            if (pc) { rc = precond_apply(ctx, p, phat, s); if (rc) return rc; pin = phat; }
+            rc = run_matvec(ctx, pin, v, true, s);
+            if (rc) return rc;
+            ++matvecs;
+            rc = device_dots(ctx, n, 1, rhat, v, ctx->hsum, nullptr, s);     // <r^, v>
+            if (rc) return rc;
+            cd dv[2];
+            rc = fetch(1, dv);
+            if (rc) return rc;
+            if (dv[0] == cd(0.0)) break;                                     // breakdown: restart
+            alpha = rho_new / dv[0];
+            celes::lincomb_kernel<<<eb, 256, 0, s>>>(n, d2(1.0), r, d2(-alpha), v, d2(0.0), nullptr, sv);   // s = r - alpha v
+            const float2* sin_ = sv;
+            if (pc) { rc = precond_apply(ctx, sv, shat, s); if (rc) return rc; sin_ = shat; }
+            rc = run_matvec(ctx, sin_, t, true, s);
+            if (rc) return rc;
+            ++matvecs; ++iterations;
+            rc = device_dots(ctx, n, 2, sv, t, ctx->hsum, nullptr, s);       // <s, t>, <t, t>   (sv and t are adjacent)
+            if (rc) return rc;
+            rc = fetch(2, dv);
+            if (rc) return rc;
+            if (dv[1].real() <= 0.0) {                                      // t = 0: s is the residual, x += alpha p^
+                celes::lincomb_kernel<<<eb, 256, 0, s>>>(n, d2(1.0), x, d2(alpha), pin, d2(0.0), nullptr, x);
+                break;
+            }
+            omega = std::conj(dv[0]) / dv[1].real();                         // <t, s> / <t, t>
+            celes::lincomb_kernel<<<eb, 256, 0, s>>>(n, d2(1.0), x, d2(alpha), pin, d2(omega), sin_, x);
+            celes::lincomb_kernel<<<eb, 256, 0, s>>>(n, d2(1.0), sv, d2(-omega), t, d2(0.0), nullptr, r);   // r = s - omega t
+            rho = rho_new;
+            rc = device_dots(ctx, n, 2, rhat, r, ctx->hsum, nullptr, s);     // <r^, r>, <r, r>   (rhat and r are adjacent)
+            if (rc) return rc;
+            rc = fetch(2, dv);
+            if (rc) return rc;
+            rho_new = dv[0];
+            const double est = std::sqrt(std::max(0.0, dv[1].real())) / fnorm;
+            push_hist(est);
+            if (est <= rtol || rho_new == cd(0.0) || omega == cd(0.0) || !std::isfinite(est)) break;
+        }
+    }
+}
+
+}  // namespace
+
+extern "C" {
+
 // Restarted GMRES (Saad & Schultz, the paper's ref. [26]) on M x = T a_in, unpreconditioned,
 // classical Gram-Schmidt with one re-orthogonalisation pass (CGS2): the j+1 inner products of a pass are ONE
 // kernel, their coefficients stay on the device for the update, and one small device->host copy per inner
@@ -444,10 +571,13 @@ int celes_solve(celes_ctx* ctx, const void* a_in_dev, void* x_dev, const celes_s
     const int restart = (o && o->restart > 0) ? o->restart : 30;
     const double rtol = (o && o->rtol > 0.0) ? o->rtol : 1e-4;
     const int max_iters = (o && o->max_iters > 0) ? o->max_iters : 1000;
-    if (method != CELES_GMRES || restart > 1024) return CELES_EINVAL;
+    const bool pc = o && o->precond == CELES_PRECOND_BLOCKDIAG;
+    if ((method != CELES_GMRES && method != CELES_BICGSTAB) || restart > 1024) return CELES_EINVAL;
+    if (o && o->precond != CELES_PRECOND_NONE && o->precond != CELES_PRECOND_BLOCKDIAG) return CELES_EINVAL;
+    if (pc && !ctx->pc_ready) return CELES_EINVAL;            // celes_precond_setup first
     cudaStream_t s = (cudaStream_t)cuda_stream;
     const auto t_start = std::chrono::steady_clock::now();
-    int rc = ensure_krylov(ctx, restart);
+    int rc = ensure_krylov(ctx, method == CELES_BICGSTAB ? std::max(restart, 8) : restart);
     if (rc) return rc;
     const long long n = (long long)ctx->N * ctx->nmax;
     const int eb = (int)std::min<long long>((n + 255) / 256, (long long)ctx->sm_count * 8);
@@ -480,6 +610,9 @@ int celes_solve(celes_ctx* ctx, const void* a_in_dev, void* x_dev, const celes_s
         return finish(CELES_OK);
     }
 
+    if (method == CELES_BICGSTAB)
+        return finish(solve_bicgstab(ctx, x, pc, rtol, max_iters, fnorm, s, iterations, matvecs, converged, rel, push_hist));
+
     std::vector<cd> Hm((size_t)(restart + 1) * restart), g(restart + 1), cs(restart), sn(restart), yv(restart);
     while (true) {
         // true residual r = rhs - M x  -> V_0
@@ -502,7 +635,13 @@ int celes_solve(celes_ctx* ctx, const void* a_in_dev, void* x_dev, const celes_s
         int j = 0;
         for (; j < restart && iterations < max_iters; ++j) {
             float2* w = V + (size_t)(j + 1) * n;
-            rc = run_matvec(ctx, V + (size_t)j * n, w, true, s);
+            if (pc) {                                          // right preconditioning: w = M (P^{-1} v_j)
+                rc = precond_apply(ctx, V + (size_t)j * n, ctx->pc_tmp, s);
+                if (rc) return finish(rc);
+                rc = run_matvec(ctx, ctx->pc_tmp, w, true, s);
+            } else {
+                rc = run_matvec(ctx, V + (size_t)j * n, w, true, s);
+            }
             if (rc) return finish(rc);
             ++matvecs; ++iterations;
             CU_TRY(cudaMemsetAsync(ctx->hsum, 0, sizeof(double2) * (j + 2), s));
@@ -546,12 +685,183 @@ int celes_solve(celes_ctx* ctx, const void* a_in_dev, void* x_dev, const celes_s
         }
         for (int i = 0; i < j; ++i) ctx->hhost[i] = make_double2(yv[i].real(), yv[i].imag());
         CU_TRY(cudaMemcpyAsync(ctx->coef, ctx->hhost, sizeof(double2) * j, cudaMemcpyHostToDevice, s));
-        if (j > 0) {
+        if (j > 0 && pc) {                                     // x += P^{-1} (V y)
+            CU_TRY(cudaMemsetAsync(ctx->tmp, 0, sizeof(float2) * n, s));
+            rc = device_axpys(ctx, n, j, 1.0, ctx->coef, V, ctx->tmp, s);
+            if (rc) return finish(rc);
+            rc = precond_apply(ctx, ctx->tmp, ctx->pc_tmp, s);
+            if (rc) return finish(rc);
+            celes::add_kernel<<<eb, 256, 0, s>>>(n, ctx->pc_tmp, x);
+        } else if (j > 0) {
             rc = device_axpys(ctx, n, j, 1.0, ctx->coef, V, x, s);
             if (rc) return finish(rc);
         }
         CU_TRY(cudaStreamSynchronize(s));      // hhost is reused by the next cycle
     }
+}
+
+int celes_partition(int N, const double* pos_xyz, const double* edge_xyz, int* group_of, int* n_groups) {
+    if (N < 1 || !pos_xyz || !edge_xyz || !group_of) return CELES_EINVAL;
+    celes::Partition part;
+    if (!celes::build_partition(N, pos_xyz, edge_xyz, part)) return CELES_EINVAL;
+    std::memcpy(group_of, part.group_of.data(), sizeof(int) * (size_t)N);
+    if (n_groups) *n_groups = part.n_groups();
+    return CELES_OK;
+}
+
+// Block-diagonal preconditioner: (1) cuboid partition, (2) blocks M_j = 1 - T W on the device,
+// (3) LU factorisation with partial pivoting (cuSOLVER getrf), here followed by the solve against the identity
+// (getrs) so that (4) applying M_j^{-1} is a batched matrix-vector product (block_gemv_kernel).
+int celes_precond_setup(celes_ctx* ctx, const double* edge_xyz, celes_precond_info* info, void* cuda_stream) {
+    if (!ctx || !edge_xyz) return CELES_EINVAL;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const auto t_start = std::chrono::steady_clock::now();
+    free_precond(ctx);
+    celes::Partition part;
+    if (!celes::build_partition(ctx->N, ctx->pos.data(), edge_xyz, part)) return CELES_EINVAL;
+    const int G = part.n_groups(), nmax = ctx->nmax, H = nmax / 2, P = 2 * ctx->lmax + 1;
+    const long long max_n = (long long)part.max_group() * nmax;
+    if (max_n * (long long)sizeof(float2) > 200 * 1024) return CELES_EINVAL;      // subset too large for one CTA's x slice
+    std::vector<long long> blk_off(G), pair_off(G + 1, 0);
+    std::vector<int> cta_group, cta_row0;
+    long long elems = 0;
+    for (int j = 0; j < G; ++j) {
+        const long long nj = part.offset[j + 1] - part.offset[j], n = nj * nmax;
+        blk_off[j] = elems;
+        elems += n * n;
+        pair_off[j + 1] = pair_off[j] + nj * nj;
+        for (long long r = 0; r < n; r += celes::kGemvRows) { cta_group.push_back(j); cta_row0.push_back((int)r); }
+    }
+    if (pair_off[G] > 0x7fffffffLL) return CELES_EINVAL;
+    std::vector<double> a5d, b5d;
+    if (!celes::build_translation_table(ctx->lmax, a5d, b5d)) return CELES_EINVAL;
+    std::vector<float> a5f(a5d.begin(), a5d.end()), b5f(b5d.begin(), b5d.end());
+
+    long long* d_pair_off = nullptr;
+    float *d_a5 = nullptr, *d_b5 = nullptr;
+    int* d_info = nullptr;
+    constexpr int kPcStreams = 8;
+    struct Lane { cudaStream_t stream = nullptr; cusolverDnHandle_t handle = nullptr; float2* lu = nullptr;
+                  int* ipiv = nullptr; void* work = nullptr; };
+    Lane lanes[kPcStreams];
+    const int nstreams = std::max(1, std::min(kPcStreams, G));
+    auto cleanup = [&](int code) {
+        cudaFree(d_pair_off); cudaFree(d_a5); cudaFree(d_b5); cudaFree(d_info);
+        for (Lane& ln : lanes) {
+            if (ln.stream) cudaStreamSynchronize(ln.stream);
+            if (ln.handle) cusolverDnDestroy(ln.handle);
+            cudaFree(ln.lu); cudaFree(ln.ipiv); cudaFree(ln.work);
+            if (ln.stream) cudaStreamDestroy(ln.stream);
+        }
+        if (code != CELES_OK) free_precond(ctx);
+        return code;
+    };
+#define PC_TRY(expr)                                                                                   \
+    do {                                                                                               \
+        cudaError_t e_ = (expr);                                                                       \
+        if (e_ != cudaSuccess) return cleanup(e_ == cudaErrorMemoryAllocation ? CELES_ENOMEM : CELES_ECUDA); \
+    } while (0)
+    PC_TRY(cudaMalloc(&ctx->pc_order, sizeof(int) * ctx->N));
+    PC_TRY(cudaMalloc(&ctx->pc_grp_offset, sizeof(int) * (G + 1)));
+    PC_TRY(cudaMalloc(&ctx->pc_blk_offset, sizeof(long long) * G));
+    PC_TRY(cudaMalloc(&ctx->pc_cta_group, sizeof(int) * cta_group.size()));
+    PC_TRY(cudaMalloc(&ctx->pc_cta_row0, sizeof(int) * cta_row0.size()));
+    PC_TRY(cudaMalloc(&ctx->pc_blocks, sizeof(float2) * (size_t)elems));
+    PC_TRY(cudaMalloc(&ctx->pc_tmp, sizeof(float2) * (size_t)ctx->N * nmax));
+    PC_TRY(cudaMalloc(&d_pair_off, sizeof(long long) * (G + 1)));
+    PC_TRY(cudaMalloc(&d_a5, sizeof(float) * a5f.size()));
+    PC_TRY(cudaMalloc(&d_b5, sizeof(float) * b5f.size()));
+    PC_TRY(cudaMalloc(&d_info, sizeof(int) * 2 * (size_t)G));
+    PC_TRY(cudaMemcpyAsync(ctx->pc_order, part.order.data(), sizeof(int) * ctx->N, cudaMemcpyHostToDevice, s));
+    PC_TRY(cudaMemcpyAsync(ctx->pc_grp_offset, part.offset.data(), sizeof(int) * (G + 1), cudaMemcpyHostToDevice, s));
+    PC_TRY(cudaMemcpyAsync(ctx->pc_blk_offset, blk_off.data(), sizeof(long long) * G, cudaMemcpyHostToDevice, s));
+    PC_TRY(cudaMemcpyAsync(ctx->pc_cta_group, cta_group.data(), sizeof(int) * cta_group.size(), cudaMemcpyHostToDevice, s));
+    PC_TRY(cudaMemcpyAsync(ctx->pc_cta_row0, cta_row0.data(), sizeof(int) * cta_row0.size(), cudaMemcpyHostToDevice, s));
+    PC_TRY(cudaMemcpyAsync(d_pair_off, pair_off.data(), sizeof(long long) * (G + 1), cudaMemcpyHostToDevice, s));
+    PC_TRY(cudaMemcpyAsync(d_a5, a5f.data(), sizeof(float) * a5f.size(), cudaMemcpyHostToDevice, s));
+    PC_TRY(cudaMemcpyAsync(d_b5, b5f.data(), sizeof(float) * b5f.size(), cudaMemcpyHostToDevice, s));
+    (void)H; (void)P;
+    // (2) assemble every block
+    {
+        const unsigned grid = (unsigned)pair_off[G];
+#define PC_ASM(L)                                                                                              \
+    celes::assemble_blocks_kernel<L><<<grid, celes::kAsmThreads, 0, s>>>(G, d_pair_off, ctx->pc_grp_offset,     \
+        ctx->pc_order, ctx->pc_blk_offset, ctx->kpos, ctx->tdiag, d_a5, d_b5, ctx->pc_blocks)
+        switch (ctx->lmax) {
+            case 1: PC_ASM(1); break;
+            case 2: PC_ASM(2); break;
+            case 3: PC_ASM(3); break;
+            case 4: PC_ASM(4); break;
+            default: return cleanup(CELES_EINVAL);
+        }
+#undef PC_ASM
+        PC_TRY(cudaGetLastError());
+    }
+    // (3) factorise and invert block by block; the blocks are independent and small against the device, so they
+    // are spread round-robin over kPcStreams streams (own cuSOLVER handle and scratch each) that fork from and join s
+    {
+        cudaEvent_t ev_fork = nullptr;
+        PC_TRY(cudaEventCreateWithFlags(&ev_fork, cudaEventDisableTiming));
+        cudaEventRecord(ev_fork, s);
+        int status = CELES_OK;
+        for (int q = 0; q < nstreams && status == CELES_OK; ++q) {
+            if (cudaStreamCreateWithFlags(&lanes[q].stream, cudaStreamNonBlocking) != cudaSuccess ||
+                cusolverDnCreate(&lanes[q].handle) != CUSOLVER_STATUS_SUCCESS ||
+                cusolverDnSetStream(lanes[q].handle, lanes[q].stream) != CUSOLVER_STATUS_SUCCESS) { status = CELES_ECUDA; break; }
+            int lwork = 0;
+            if (cudaMalloc(&lanes[q].lu, sizeof(float2) * (size_t)(max_n * max_n)) != cudaSuccess ||
+                cudaMalloc(&lanes[q].ipiv, sizeof(int) * (size_t)max_n) != cudaSuccess) { status = CELES_ENOMEM; break; }
+            if (cusolverDnCgetrf_bufferSize(lanes[q].handle, (int)max_n, (int)max_n, (cuComplex*)lanes[q].lu, (int)max_n,
+                                            &lwork) != CUSOLVER_STATUS_SUCCESS) { status = CELES_ECUDA; break; }
+            if (cudaMalloc(&lanes[q].work, sizeof(cuComplex) * (size_t)std::max(lwork, 1)) != cudaSuccess) { status = CELES_ENOMEM; break; }
+            cudaStreamWaitEvent(lanes[q].stream, ev_fork, 0);
+        }
+        for (int j = 0; j < G && status == CELES_OK; ++j) {
+            Lane& ln = lanes[j % nstreams];
+            const int n = (part.offset[j + 1] - part.offset[j]) * nmax;
+            float2* Mj = ctx->pc_blocks + blk_off[j];
+            if (cudaMemcpyAsync(ln.lu, Mj, sizeof(float2) * (size_t)n * n, cudaMemcpyDeviceToDevice, ln.stream) != cudaSuccess) status = CELES_ECUDA;
+            const int ib = (int)std::min<long long>(((long long)n * n + 255) / 256, (long long)ctx->sm_count * 8);
+            celes::set_identity_kernel<<<ib, 256, 0, ln.stream>>>(n, Mj);
+            if (cusolverDnCgetrf(ln.handle, n, n, (cuComplex*)ln.lu, n, (cuComplex*)ln.work, ln.ipiv, d_info + 2 * j) !=
+                CUSOLVER_STATUS_SUCCESS) status = CELES_ECUDA;
+            if (cusolverDnCgetrs(ln.handle, CUBLAS_OP_N, n, n, (const cuComplex*)ln.lu, n, ln.ipiv, (cuComplex*)Mj, n,
+                                 d_info + 2 * j + 1) != CUSOLVER_STATUS_SUCCESS) status = CELES_ECUDA;
+        }
+        for (int q = 0; q < nstreams; ++q) {                   // join
+            if (!lanes[q].stream) continue;
+            cudaEvent_t ev = nullptr;
+            if (cudaEventCreateWithFlags(&ev, cudaEventDisableTiming) == cudaSuccess) {
+                cudaEventRecord(ev, lanes[q].stream);
+                cudaStreamWaitEvent(s, ev, 0);
+                cudaEventDestroy(ev);
+            } else {
+                cudaStreamSynchronize(lanes[q].stream);
+            }
+        }
+        cudaEventDestroy(ev_fork);
+        if (status != CELES_OK) { cudaStreamSynchronize(s); return cleanup(status); }
+    }
+    std::vector<int> infos(2 * (size_t)G);
+    PC_TRY(cudaMemcpyAsync(infos.data(), d_info, sizeof(int) * infos.size(), cudaMemcpyDeviceToHost, s));
+    PC_TRY(cudaStreamSynchronize(s));
+#undef PC_TRY
+    for (int v : infos) if (v != 0) return cleanup(CELES_ECUDA);     // singular block or bad argument
+    ctx->pc_groups = G; ctx->pc_max_n = (int)max_n; ctx->pc_ctas = (int)cta_group.size(); ctx->pc_elems = elems;
+    ctx->pc_ready = true;
+    cudaFuncSetAttribute(celes::block_gemv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(max_n * sizeof(float2)));
+    if (info) {
+        info->n_groups = G;
+        info->max_group_spheres = part.max_group();
+        info->block_bytes = elems * (long long)sizeof(float2);
+        info->seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_start).count();
+    }
+    return cleanup(CELES_OK);
+}
+
+int celes_precond_apply(celes_ctx* ctx, const void* v_dev, void* z_dev, void* cuda_stream) {
+    if (!ctx || !v_dev || !z_dev || v_dev == z_dev || !ctx->pc_ready) return CELES_EINVAL;
+    return precond_apply(ctx, (const float2*)v_dev, (float2*)z_dev, (cudaStream_t)cuda_stream);
 }
 
 void celes_destroy(celes_ctx* ctx) { free_ctx(ctx); }

@@ -97,4 +97,17 @@ __global__ void sub_kernel(long long n, const float2* __restrict__ a, const floa
         out[t] = make_float2(a[t].x - b[t].x, a[t].y - b[t].y);
 }
 
+// out = a x + b y + c z  (complex scalars by value; y, z may be nullptr when their scalar is unused; out may alias
+// any input).  The vector updates of BiCGSTAB.
+__global__ void lincomb_kernel(long long n, double2 a, const float2* __restrict__ x, double2 b, const float2* y,
+                               double2 c, const float2* z, float2* out) {
+    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += (long long)gridDim.x * blockDim.x) {
+        const float2 xv = x[t];
+        double r = a.x * xv.x - a.y * xv.y, i = a.x * xv.y + a.y * xv.x;
+        if (y != nullptr) { const float2 v = y[t]; r += b.x * v.x - b.y * v.y; i += b.x * v.y + b.y * v.x; }
+        if (z != nullptr) { const float2 v = z[t]; r += c.x * v.x - c.y * v.y; i += c.x * v.y + c.y * v.x; }
+        out[t] = make_float2((float)r, (float)i);
+    }
+}
+
 }  // namespace celes

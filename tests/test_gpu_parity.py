@@ -227,3 +227,72 @@ def test_c5_full_size_solve():
     rhs = T * a_in[recv]
     res = rhs - (xg[recv] - T * Wx)
     assert np.linalg.norm(res) / np.linalg.norm(rhs) <= 3e-4
+
+
+def test_precond_apply_matches_oracle_block_solve():
+    """celes_precond_apply against the oracle's block-by-block dense solve (PAPER.md:109-116) on a C3-shaped slab;
+    the blocks are assembled and inverted in FP32, so the tolerance is the solve tolerance."""
+    w = workloads.scaled(workloads.C3, 400)
+    pos, rad, q, ctx, b = make(w)
+    edge = [1200.0, 1500.0, 0.0]
+    info = celes.celes_precond_setup(ctx, edge)
+    groups = orc.cuboid_partition(pos, edge)
+    assert info["n_groups"] == len(groups) and info["max_group_spheres"] == max(len(g) for g in groups)
+    assert info["block_bytes"] == 8 * sum((len(g) * w.nmax) ** 2 for g in groups)
+    z = celes.celes_precond_apply(ctx, torch.from_numpy(b).cuda()).cpu().numpy()
+    qo = orc.mie_q(w.lmax, w.k, rad, workloads.N_SPHERE)
+    ref = orc.precond_apply(pos, w.k, w.lmax, qo, edge, b)
+    assert rel(z, ref) <= SOLVE_TOL
+
+
+@pytest.mark.parametrize("lmax", [1, 2, 4])
+def test_precond_apply_every_lmax(lmax):
+    import dataclasses
+    w = dataclasses.replace(workloads.scaled(workloads.C2, 60), lmax=lmax)
+    pos, rad, q, ctx, b = make(w)
+    celes.celes_precond_setup(ctx, 900.0)
+    z = celes.celes_precond_apply(ctx, torch.from_numpy(b).cuda()).cpu().numpy()
+    qo = orc.mie_q(w.lmax, w.k, rad, workloads.N_SPHERE)
+    assert rel(z, orc.precond_apply(pos, w.k, w.lmax, qo, 900.0, b)) <= SOLVE_TOL
+
+
+def test_preconditioned_solve_same_solution_fewer_iterations():
+    """Right-preconditioned GMRES: same solution as the oracle's tight solve, fewer iterations
+    than the unpreconditioned solve; asking for the preconditioner before celes_precond_setup is an error."""
+    w = workloads.scaled(workloads.C5, 600)
+    pos, rad, q, ctx, _ = make(w)
+    qo = orc.mie_q(w.lmax, w.k, rad, workloads.N_SPHERE)
+    a_in = orc.plane_wave_a_in(pos, w.k, w.lmax)
+    a_dev = torch.from_numpy(a_in.astype(np.complex64)).cuda()
+    x = torch.zeros(w.N, w.nmax, dtype=torch.complex64, device="cuda")
+    with pytest.raises(celes.CelesError):
+        celes.celes_solve(ctx, a_dev, x, precond=True)
+    plain = celes.celes_solve(ctx, a_dev, x, restart=30, rtol=1e-4)
+    x_plain = x.cpu().numpy()
+    celes.celes_precond_setup(ctx, [1500.0, 1500.0, 0.0])
+    x.zero_()
+    pre = celes.celes_solve(ctx, a_dev, x, restart=30, rtol=1e-4, precond=True)
+    assert plain["converged"] and pre["converged"] and pre["rel_residual"] <= 1e-4
+    assert pre["iterations"] < plain["iterations"]
+    xref, _ = orc.solve_gmres(pos, w.k, w.lmax, qo, a_in, rtol=1e-10)
+    assert rel(x.cpu().numpy(), xref) <= SOLVE_TOL
+    assert rel(x_plain, xref) <= SOLVE_TOL
+
+
+@pytest.mark.parametrize("precond", [False, True])
+def test_bicgstab_same_solution(precond):
+    """The paper's second solver: BiCGSTAB reaches the same unique solution of eq. (8) as the
+    oracle's tight solve, with and without the block-diagonal preconditioner; the TRUE residual decides."""
+    w = workloads.scaled(workloads.C2, 300)
+    pos, rad, q, ctx, _ = make(w)
+    qo = orc.mie_q(w.lmax, w.k, rad, workloads.N_SPHERE)
+    a_in = orc.plane_wave_a_in(pos, w.k, w.lmax)
+    xref, _ = orc.solve_gmres(pos, w.k, w.lmax, qo, a_in, rtol=1e-10)
+    if precond:
+        celes.celes_precond_setup(ctx, 700.0)
+    x = torch.zeros(w.N, w.nmax, dtype=torch.complex64, device="cuda")
+    info = celes.celes_solve(ctx, torch.from_numpy(a_in.astype(np.complex64)).cuda(), x, rtol=1e-4, method="bicgstab",
+                             precond=precond)
+    assert info["converged"] and info["rel_residual"] <= 1e-4, info
+    assert info["matvecs"] >= 2 * info["iterations"]
+    assert rel(x.cpu().numpy(), xref) <= SOLVE_TOL

@@ -152,3 +152,18 @@ def test_workloads_are_seeded_and_valid():
     b = workloads.gaussian_coefficients(w.N, w.nmax, w.seed_b)
     assert b.dtype == np.complex64 and b.shape == (50, 30)
     assert abs(np.mean(np.abs(b) ** 2) - 1.0) < 0.1
+
+
+def test_partition_matches_oracle_cuboids():
+    """celes_partition (host side of celes_precond_setup) against the oracle's cuboid partition:
+    same subsets, same numbering (lexicographic cuboid order)."""
+    w = workloads.scaled(workloads.C3, 1500)
+    pos, _ = workloads.positions(w)
+    for edge in ([1000.0, 1500.0, 0.0], [800.0, 800.0, 100.0], [0.0, 0.0, 0.0], 2500.0):
+        g, n = celes.celes_partition(pos, edge)
+        ref = orc.cuboid_partition(pos, edge)
+        assert n == len(ref)
+        for j, idx in enumerate(ref):
+            assert np.all(g[idx] == j)
+    with pytest.raises(celes.CelesError):
+        celes.celes_partition(np.array([[np.nan, 0.0, 0.0]]), 1.0)

@@ -332,3 +332,49 @@ def test_p11_matvec_equals_dense_assembly_and_gmres_equals_lu():
     x_it, info = o.solve_gmres(pos, w.k, w.lmax, q, a_in, rtol=1e-11, restart=40)
     assert info["rel_residual"] <= 1e-11
     assert _rel(x_it, x_lu) < 1e-9
+
+
+# --------------------------------------------------------------------------- P13 block-diagonal preconditioner
+def test_p13_preconditioner_limits_and_partition_brute_force():
+    """PAPER.md:109-116.  (a) one cuboid holding every sphere: the preconditioner IS M^{-1} (dense LU of eq. 8);
+    (b) cuboids so small that every sphere is alone: M_j = 1 (W^{ii} = 0), z = v; (c) the partition against a
+    brute-force pairwise statement of "same cuboid"; (d) two clusters far apart cut between them: M z = v up to
+    the weak far coupling, and exactly M_jj z_j = v_j block by block."""
+    from paper_1706_02145_b200 import workloads as wl
+    w = wl.scaled(wl.C2, 20)
+    pos, rad = wl.positions(w)
+    q = o.mie_q(w.lmax, w.k, rad, wl.N_SPHERE)
+    n = o.nmax_of(w.lmax)
+    v = wl.gaussian_coefficients(w.N, w.nmax, 77).astype(np.complex128)
+    M = o.dense_system_matrix(pos, w.k, w.lmax, q)
+    # (a)
+    z = o.precond_apply(pos, w.k, w.lmax, q, [0.0, 0.0, 0.0], v)
+    assert _rel(M @ z.reshape(-1), v.reshape(-1)) < 1e-11
+    # (b)
+    assert np.array_equal(o.precond_apply(pos, w.k, w.lmax, q, 1.0, v), v)
+    # (c)
+    edge = np.array([700.0, 900.0, 0.0])
+    groups = o.cuboid_partition(pos, edge)
+    label = np.empty(w.N, dtype=int)
+    for j, idx in enumerate(groups):
+        label[idx] = j
+    assert sorted(np.concatenate(groups).tolist()) == list(range(w.N))
+    lo = pos.min(axis=0)
+    for i in range(w.N):
+        for ip in range(w.N):
+            same = all(edge[a] <= 0 or int((pos[i, a] - lo[a]) // edge[a]) == int((pos[ip, a] - lo[a]) // edge[a])
+                       for a in range(3))
+            assert same == (label[i] == label[ip])
+    # (d)
+    far = pos.copy()
+    half = pos[:, 0] > np.median(pos[:, 0])
+    far[half, 0] += 4.0e5                                      # second cluster 400 um away
+    span = far[:, 0].max() - far[:, 0].min()
+    gr = o.cuboid_partition(far, [0.6 * span, 0.0, 0.0])
+    assert len(gr) == 2 and set(gr[1].tolist()) == set(np.nonzero(half)[0].tolist())
+    Mf = o.dense_system_matrix(far, w.k, w.lmax, q)
+    zf = o.precond_apply(far, w.k, w.lmax, q, [0.6 * span, 0.0, 0.0], v)
+    for idx in gr:
+        rows = (idx[:, None] * n + np.arange(n)[None, :]).reshape(-1)
+        assert _rel(Mf[np.ix_(rows, rows)] @ zf[idx].reshape(-1), v[idx].reshape(-1)) < 1e-11
+    assert _rel(Mf @ zf.reshape(-1), v.reshape(-1)) < 1e-2      # coupling ~ 1/(k d) across 400 um

@@ -3,12 +3,13 @@
 FP64, CPU, plain.  Each function cites the passage of PAPER.md it restates.  The N^2 coupling
 sum itself lives in ``celes_oracle.cpp`` (same directory) and is reached through ctypes; this
 file adds what surrounds it on the hot path: the sphere T-matrix (B.1-B.3), the system
-operator of eqs. (8)-(9), the plane-wave right-hand side (A.13-A.14), a reference solve, and
+operator of eqs. (8)-(9), the plane-wave right-hand side (A.13-A.14), a reference solve, the
+block-diagonal preconditioner of PAPER.md:109-116 (cuboid partition, block-by-block dense solve), and
 the SVWF / PVWF evaluators (A.2, A.4) that the pins in tests/test_oracle_pins.py use for the
 brute-force addition-theorem check.
 
 Nothing in here imports, reads or shares anything with ``paper_1706_02145_b200/``.
-Pins: see tests/test_oracle_pins.py (P1-P11 of DESIGN.md).  Nothing is "parity unpinned".
+Pins: see tests/test_oracle_pins.py (P1-P11, P13 of DESIGN.md).  Nothing is "parity unpinned".
 """
 from __future__ import annotations
 

@@ -120,6 +120,23 @@ def measured_peaks() -> dict:
         return {}
 
 
+def max_over_ranks(value: float, world: int, device) -> float:
+    """Slowest rank's value (replicas only: no data-path collective; this all-reduce of one
+    scalar is the measurement, not the method).  Works with nccl (CUDA tensor) and gloo (CPU tensor)."""
+    if world <= 1:
+        return float(value)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_throughput(pairs_per_replica: int, steps: int, world: int, slowest_total_ms: float) -> float:
+    """Whole-job pair translations per second of `world` independent replicas timed by the slowest one."""
+    return world * pairs_per_replica * steps / (slowest_total_ms * 1e-3)
+
+
 def oracle_sample_rate(w, pos, b, seconds: float):
     """Times the oracle (as it stands) on whole receivers of workload w until about `seconds` of CPU work."""
     from oracle import celes_oracle as orc
@@ -291,13 +308,9 @@ def main():
     barrier()
     clocks = sampler.stop()
     step_ms = [a.elapsed_time(c) for a, c in ev]
-    total_ms = float(sum(step_ms))
-    t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    total_ms = float(t.item())
+    total_ms = max_over_ranks(float(sum(step_ms)), world, "cuda")
     ms_per_step = total_ms / args.steps
-    value = world * pairs * args.steps / (total_ms * 1e-3)
+    value = job_throughput(pairs, args.steps, world, total_ms)
 
     # end to end: pinned host buffers through the C ABI's host entry point, copies inside the timed region
     bh = torch.from_numpy(b_host).pin_memory()
@@ -309,11 +322,8 @@ def main():
     for s in range(args.steps):
         celes.celes_coupling_matvec_host(ctx, bh_np, yh_np)
     barrier()
-    e2e_s = time.perf_counter() - t0
-    te = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(te, op=dist.ReduceOp.MAX)
-    e2e_value = world * pairs * args.steps / float(te.item())
+    e2e_s = max_over_ranks(time.perf_counter() - t0, world, "cuda")
+    e2e_value = job_throughput(pairs, args.steps, world, e2e_s * 1e3)
 
     if rank == 0:
         peaks = measured_peaks()

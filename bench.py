@@ -57,6 +57,8 @@ def parse():
                     help="time celes_solve (plane wave, GMRES(30), rtol 1e-4) on the workload instead (config 5: --workload C5)")
     ap.add_argument("--precond-edge", type=float, default=0.0,
                     help="with --solve: lateral edge (nm) of the cuboids of the block-diagonal preconditioner (0 = none)")
+    ap.add_argument("--hankel", default="registers", choices=["registers", "table"],
+                    help="h_p(kd) in registers (default) or from the paper's lookup table (PAPER.md:130)")
     ap.add_argument("--method", default="gmres", choices=["gmres", "bicgstab"], help="with --solve")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=20.0, help="CPU work of the cpu_baseline sample")
@@ -277,7 +279,7 @@ def main():
     q = fields.mie_coefficients(w.lmax, w.k, rad, workloads.N_SPHERE)
     b_host = workloads.gaussian_coefficients(w.N, w.nmax, w.seed_b + rank)
     t0 = time.perf_counter()
-    ctx = celes.celes_setup(pos, rad, q, w.k, w.lmax, translation=args.translation)
+    ctx = celes.celes_setup(pos, rad, q, w.k, w.lmax, translation=args.translation, hankel=args.hankel)
     setup_s = time.perf_counter() - t0
     cfg = celes.celes_launch_config(ctx)
     b = torch.from_numpy(b_host).cuda()
@@ -342,7 +344,7 @@ def main():
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": f"{w.name}: N={w.N} lmax={w.lmax} R=100nm n=1.52 lambda=550nm slab RSA ff=0.3",
                        "pairs_per_step": pairs, "l2": "flushed between timed iterations (256 MiB write)",
-                       "launch": cfg, "parallelism": "replicas only" if world > 1 else "single GPU",
+                       "launch": cfg, "hankel": args.hankel, "parallelism": "replicas only" if world > 1 else "single GPU",
                        "setup_s": setup_s, "step_ms_min": float(min(step_ms)), "step_ms_median": float(np.median(step_ms))},
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(b_host.nbytes),

@@ -52,7 +52,15 @@ typedef struct celes_options {
                               CELES_TRANSLATION_DIRECT sums (A.6)-(A.8) term by term;
                               CELES_TRANSLATION_ROTATED_SCALAR is the rotated scheme in scalar FP32 instructions.
                               Same result up to FP32 rounding. */
+    int hankel;            /* how h_p^(1)(kd) is obtained per pair: CELES_HANKEL_REGISTERS (default) evaluates e^{ikd}
+                              and the upward recurrence in registers; CELES_HANKEL_TABLE is the paper's scheme
+                              (PAPER.md:130): a lookup table over the radial distance with spacing hankel_dr, built by
+                              celes_setup on the device, interpolated with cubic (Hermite) splines in the kernel.
+                              Only with CELES_TRANSLATION_ROTATED. */
+    double hankel_dr;      /* table spacing Delta r in the length unit U; 0 = default 1.0 (1 nm in PAPER.md:140) */
 } celes_options;
+#define CELES_HANKEL_REGISTERS 0
+#define CELES_HANKEL_TABLE     1
 #define CELES_TRANSLATION_ROTATED        0
 #define CELES_TRANSLATION_DIRECT         1
 #define CELES_TRANSLATION_ROTATED_SCALAR 2
@@ -93,8 +101,10 @@ typedef struct celes_solve_info {
  *   radii    host, [N] double, R_i; used only to verify that spheres are disjoint (needed for |r| < |d| in A.5).
  *   mie_q    host, [N][2][lmax] complex128 interleaved: Q^i_{tau,l} of (B.2)-(B.3).
  *   k        background wavenumber n_0 omega / c > 0.
- * Builds on the device: k-scaled FP64 centres, the T diagonal, and the a5/b5 translation-coefficient table
- * (PAPER.md:129, 258-267).  Copies everything it needs; the host arrays may be freed afterwards.
+ * Builds on the device: k-scaled FP64 centres, the T diagonal and, if asked for, the spherical-Hankel lookup table
+ * (PAPER.md:130); the a5/b5 translation coefficients are immediates of the generated pair
+ * bodies and a device table for the preconditioner's block assembly.  Copies everything it needs; the host arrays
+ * may be freed afterwards.
  * On success *out is a new context; on error *out is NULL. */
 int celes_setup(celes_ctx** out, int N, int lmax, const double* pos_xyz, const double* radii,
                 const double* mie_q, double k, const celes_options* opt, void* cuda_stream);

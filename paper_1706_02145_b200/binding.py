@@ -37,7 +37,7 @@ class CelesError(RuntimeError):
 
 class celes_options(ctypes.Structure):
     _fields_ = [("emitter_tile", ctypes.c_int), ("emitter_splits", ctypes.c_int), ("skip_overlap_check", ctypes.c_int),
-                ("translation", ctypes.c_int)]
+                ("translation", ctypes.c_int), ("hankel", ctypes.c_int), ("hankel_dr", ctypes.c_double)]
 
 
 class celes_solve_opts(ctypes.Structure):
@@ -134,7 +134,8 @@ class Context:
 
 
 def celes_setup(pos_xyz, radii, mie_q, k: float, lmax: int, *, emitter_tile: int = 0, emitter_splits: int = 0,
-                skip_overlap_check: bool = False, translation: str = "rotated", stream=None) -> Context:
+                skip_overlap_check: bool = False, translation: str = "rotated", hankel: str = "registers",
+                hankel_dr: float = 0.0, stream=None) -> Context:
     """celes_setup of include/celes.h.  pos_xyz [N,3] float64, radii [N] float64, mie_q [N,2,lmax] complex128 (host)."""
     pos = np.ascontiguousarray(pos_xyz, dtype=np.float64)
     rad = np.ascontiguousarray(radii, dtype=np.float64)
@@ -145,7 +146,7 @@ def celes_setup(pos_xyz, radii, mie_q, k: float, lmax: int, *, emitter_tile: int
     if translation not in TRANSLATIONS:
         raise ValueError("translation: one of " + ", ".join(TRANSLATIONS))
     opt = celes_options(int(emitter_tile), int(emitter_splits), int(bool(skip_overlap_check)),
-                        TRANSLATIONS[translation])
+                        TRANSLATIONS[translation], {"registers": 0, "table": 1}[hankel], float(hankel_dr))
     h = ctypes.c_void_p()
     import torch
     s = _stream(stream) if torch.cuda.is_available() else 0

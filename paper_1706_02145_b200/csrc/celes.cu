@@ -35,6 +35,8 @@ struct celes_ctx {
     std::vector<double> pos;     // host copy of the centres [N][3] (partition of the preconditioner)
     double* kpos = nullptr;      // [N][3] FP64, k * r_i
     float2* tdiag = nullptr;     // [N][nmax] T diagonal Q^i_{tau,l} expanded over m (B.1)
+    float4* htab = nullptr;      // Hankel lookup table [nodes][2 lmax + 1] (CELES_HANKEL_TABLE), else null
+    HankelTable htab_desc = {nullptr, 0.0f, 0.0f, 0};
     float2* bpm = nullptr;       // [N][nmax] work: [b_+ | b_-]
     float2* ypart = nullptr;     // [splits][N][nmax] work: partial sums of the emitter splits
     // Krylov work space (allocated on the first celes_solve)
@@ -71,21 +73,35 @@ using celes::kBlock;
         }                                             \
     } while (0)
 
-template <int LMAX, int ROT>
-int launch_coupling_t(const celes_ctx* c, cudaStream_t s) {
+template <int LMAX, int ROT, bool TAB>
+int launch_coupling_tt(const celes_ctx* c, cudaStream_t s) {
     const size_t smem = celes::coupling_smem_bytes<LMAX>(c->etile);
     dim3 grid(c->rblocks, c->splits);
-    celes::coupling_kernel<LMAX, ROT><<<grid, kBlock, smem, s>>>(c->N, c->chunk, c->etile, c->kpos, c->bpm, c->ypart);
+    celes::coupling_kernel<LMAX, ROT, TAB><<<grid, kBlock, smem, s>>>(c->N, c->chunk, c->etile, c->htab_desc, c->kpos,
+                                                                      c->bpm, c->ypart);
     return cudaGetLastError() == cudaSuccess ? CELES_OK : CELES_ECUDA;
+}
+
+template <int LMAX, int ROT, bool TAB>
+int prepare_coupling_tt(celes_ctx* c, int* ctas_per_sm) {
+    const size_t smem = celes::coupling_smem_bytes<LMAX>(c->etile);
+    c->coupling_smem = smem;
+    CU_TRY(cudaFuncSetAttribute(celes::coupling_kernel<LMAX, ROT, TAB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, celes::coupling_kernel<LMAX, ROT, TAB>, kBlock, smem));
+    return CELES_OK;
+}
+
+// the table look-up exists for the default (packed rotated) body only
+template <int LMAX, int ROT>
+int launch_coupling_t(const celes_ctx* c, cudaStream_t s) {
+    if constexpr (ROT == celes::kRotated) { if (c->htab) return launch_coupling_tt<LMAX, ROT, true>(c, s); }
+    return launch_coupling_tt<LMAX, ROT, false>(c, s);
 }
 
 template <int LMAX, int ROT>
 int prepare_coupling_t(celes_ctx* c, int* ctas_per_sm) {
-    const size_t smem = celes::coupling_smem_bytes<LMAX>(c->etile);
-    c->coupling_smem = smem;
-    CU_TRY(cudaFuncSetAttribute(celes::coupling_kernel<LMAX, ROT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, celes::coupling_kernel<LMAX, ROT>, kBlock, smem));
-    return CELES_OK;
+    if constexpr (ROT == celes::kRotated) { if (c->htab) return prepare_coupling_tt<LMAX, ROT, true>(c, ctas_per_sm); }
+    return prepare_coupling_tt<LMAX, ROT, false>(c, ctas_per_sm);
 }
 
 #define CELES_DISPATCH(fn, ...)                                                                              \
@@ -172,7 +188,7 @@ void free_precond(celes_ctx* c) {
 void free_ctx(celes_ctx* c) {
     if (!c) return;
     free_precond(c);
-    cudaFree(c->kpos); cudaFree(c->tdiag); cudaFree(c->bpm); cudaFree(c->ypart);
+    cudaFree(c->kpos); cudaFree(c->tdiag); cudaFree(c->bpm); cudaFree(c->ypart); cudaFree(c->htab);
     cudaFree(c->V); cudaFree(c->rhs); cudaFree(c->tmp); cudaFree(c->partial); cudaFree(c->coef); cudaFree(c->hsum);
     if (c->hhost) cudaFreeHost(c->hhost);
     delete c;
@@ -350,6 +366,10 @@ int celes_setup(celes_ctx** out, int N, int lmax, const double* pos_xyz, const d
     if (!skip && !spheres_disjoint(N, pos_xyz, radii)) return CELES_EINVAL;
     if (opt && (opt->emitter_tile < 0 || opt->emitter_splits < 0 || opt->emitter_tile > 128)) return CELES_EINVAL;
     if (opt && (opt->translation < 0 || opt->translation > CELES_TRANSLATION_ROTATED_SCALAR)) return CELES_EINVAL;
+    const bool table = opt && opt->hankel == CELES_HANKEL_TABLE;
+    if (opt && opt->hankel != CELES_HANKEL_REGISTERS && opt->hankel != CELES_HANKEL_TABLE) return CELES_EINVAL;
+    if (table && (opt->translation != CELES_TRANSLATION_ROTATED || !(opt->hankel_dr >= 0.0) || !std::isfinite(opt->hankel_dr)))
+        return CELES_EINVAL;
 
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); return CELES_ECUDA; }
@@ -366,6 +386,43 @@ int celes_setup(celes_ctx** out, int N, int lmax, const double* pos_xyz, const d
     c->etile = (opt && opt->emitter_tile > 0) ? opt->emitter_tile : 32;
     c->variant = opt ? opt->translation : CELES_TRANSLATION_ROTATED;
     c->rblocks = (N + kBlock - 1) / kBlock;
+    if (table) {
+        // S2: h_p^(1)(k r) for r from the smallest possible centre distance (two touching spheres of
+        // the smallest radius; spheres are disjoint) to the diagonal of the centres' bounding box, spacing dr; FP64
+        // on the host, stored FP32 with the derivative (h_p' = h_{p-1} - (p+1)/x h_p, h_0' = -h_1) for Hermite cubics.
+        const double dr = opt->hankel_dr > 0.0 ? opt->hankel_dr : 1.0;
+        double rmin = radii[0], lo[3] = {pos_xyz[0], pos_xyz[1], pos_xyz[2]}, hi[3] = {pos_xyz[0], pos_xyz[1], pos_xyz[2]};
+        for (int i = 0; i < N; ++i) {
+            rmin = std::min(rmin, radii[i]);
+            for (int a = 0; a < 3; ++a) { lo[a] = std::min(lo[a], pos_xyz[3 * i + a]); hi[a] = std::max(hi[a], pos_xyz[3 * i + a]); }
+        }
+        const double dmin = 2.0 * rmin;
+        const double dmax = std::sqrt((hi[0] - lo[0]) * (hi[0] - lo[0]) + (hi[1] - lo[1]) * (hi[1] - lo[1]) + (hi[2] - lo[2]) * (hi[2] - lo[2]));
+        const double nodes_d = std::ceil(std::max(0.0, dmax - dmin) / dr) + 2.0;
+        const int P = 2 * lmax + 1;
+        if (!(nodes_d * P * sizeof(float4) <= 2.0e9)) return fail(CELES_EINVAL);           // table spacing too fine
+        const int nodes = (int)nodes_d;
+        std::vector<float4> tab((size_t)nodes * P);
+        for (int j = 0; j < nodes; ++j) {
+            const double x = k * (dmin + j * dr), dxs = k * dr;
+            typedef std::complex<double> cd;
+            const cd e = std::exp(cd(0.0, x));
+            cd h[16];
+            h[0] = cd(0.0, -1.0) * e / x;
+            h[1] = -e * cd(x, 1.0) / (x * x);
+            for (int p = 1; p + 1 < P; ++p) h[p + 1] = (2.0 * p + 1.0) / x * h[p] - h[p - 1];
+            for (int p = 0; p < P; ++p) {
+                const cd d = p == 0 ? -h[1] : h[p - 1] - (p + 1.0) / x * h[p];
+                tab[(size_t)j * P + p] = make_float4((float)h[p].real(), (float)h[p].imag(), (float)(dxs * d.real()), (float)(dxs * d.imag()));
+            }
+        }
+        if (cudaMalloc(&c->htab, sizeof(float4) * tab.size()) != cudaSuccess) return fail(CELES_ENOMEM);
+        if (cudaMemcpy(c->htab, tab.data(), sizeof(float4) * tab.size(), cudaMemcpyHostToDevice) != cudaSuccess) return fail(CELES_ECUDA);
+        c->htab_desc.nodes = c->htab;
+        c->htab_desc.x0 = (float)(k * dmin);
+        c->htab_desc.inv_dx = (float)(1.0 / (k * dr));
+        c->htab_desc.last = nodes - 1;
+    }
     int ctas_per_sm = 1;
     rc = prepare_coupling(c, &ctas_per_sm);
     if (rc) return fail(rc);

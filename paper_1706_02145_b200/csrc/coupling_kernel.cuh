@@ -123,8 +123,8 @@ constexpr size_t coupling_smem_bytes(int etile) {
 // grid = (ceil(N / kBlock), splits).  CTA (bx, by) translates emitters [by*chunk, min(N, (by+1)*chunk)) to
 // receivers bx*kBlock + tid and writes its partial sums to ypart[by][receiver][q].
 //   kpos  [N][3] FP64: k * r_i.  The subtraction r_i - r_i' is done in FP64, everything after it in FP32.
-template <int LMAX, int VARIANT>
-__global__ void CELES_COUPLING_BOUNDS coupling_kernel(int N, int chunk, int etile,
+template <int LMAX, int VARIANT, bool TABLE>
+__global__ void CELES_COUPLING_BOUNDS coupling_kernel(int N, int chunk, int etile, HankelTable htab,
                                                           const double* __restrict__ kpos,
                                                           const float2* __restrict__ bpm,
                                                           float2* __restrict__ ypart) {
@@ -164,7 +164,7 @@ __global__ void CELES_COUPLING_BOUNDS coupling_kernel(int N, int chunk, int etil
             const float dz = (float)(zi - spos[3 * e + 2]);
             const float2* be = sb + e * NMAX;
             auto bload = [be](int q) { return be[q]; };        // same address in every lane: LDS broadcast
-            pair_translate<LMAX, VARIANT>(dx, dy, dz, bload, yacc);
+            pair_translate<LMAX, VARIANT, TABLE>(dx, dy, dz, htab, bload, yacc);
         }
     }
     if (active) {

@@ -51,11 +51,19 @@ constexpr int kDirect = 1;          // term-by-term sum of (A.6)-(A.8)
 constexpr int kRotatedScalar = 2;   // scalar-FFMA rotate / axial-translate / rotate
 }  // namespace celes
 
+// Spherical-Hankel lookup table of the paper's scheme: node j holds, for p = 0..2 lmax,
+// (Re h_p, Im h_p, dx Re h_p', dx Im h_p') at x_j = x0 + j dx; cubic Hermite interpolation between two nodes.
+struct HankelTable {
+    const float4* nodes;   // [n_nodes][P]
+    float x0, inv_dx;
+    int last;              // index of the last node
+};
+
 // dx, dy, dz: components of k (r_i - r_i') (dimensionless), already rounded to FP32 AFTER the subtraction
 // was done in FP64 (coordinate rounding is the dominant FP32 error otherwise).
 // bload(q): emitter coefficient q in the variant's work basis;  yacc: accumulator policy of the receiver.
-template <int LMAX, int VARIANT, class BLoad, class YAcc>
-CELES_DEVICE void pair_translate(float dx, float dy, float dz, const BLoad& bload, YAcc& yacc) {
+template <int LMAX, int VARIANT, bool TABLE, class BLoad, class YAcc>
+CELES_DEVICE void pair_translate(float dx, float dy, float dz, const HankelTable& htab, const BLoad& bload, YAcc& yacc) {
     constexpr int P = 2 * LMAX + 1;
     // ---- H2 geometry: spherical coordinates of d
     const float rho2 = fmaf(dx, dx, dy * dy);
@@ -70,6 +78,22 @@ CELES_DEVICE void pair_translate(float dx, float dy, float dz, const BLoad& bloa
     const float st = rho2 * rhoinv * rinv;
     // ---- H3 radial functions: h_0 = -i e^{ix}/x, h_1 = -e^{ix}(x+i)/x^2, upward recurrence (stable relative
     // to |h_p| because the Neumann part dominates wherever the Bessel part's recurrence is unstable)
+    if constexpr (VARIANT == celes::kRotated && TABLE) {    // the paper's table look-up
+        const float t = (x - htab.x0) * htab.inv_dx;
+        const int j = min(max((int)t, 0), htab.last - 1);
+        const float u = t - (float)j, v = 1.0f - u;
+        const float h00 = (1.0f + 2.0f * u) * v * v, h10 = u * v * v, h01 = u * u * (3.0f - 2.0f * u), h11 = -u * u * v;
+        const float4* n0 = htab.nodes + (size_t)j * P;
+        float2 h[P];
+#pragma unroll
+        for (int p = 0; p < P; ++p) {
+            const float4 a = __ldg(n0 + p), b = __ldg(n0 + P + p);
+            h[p] = fma2(bc2(h11), make_float2(b.z, b.w), fma2(bc2(h01), make_float2(b.x, b.y),
+                   fma2(bc2(h10), make_float2(a.z, a.w), mul2(bc2(h00), make_float2(a.x, a.y)))));
+        }
+        PairBodyPk<LMAX>::run(h, ct, st, cph, sph, bload, yacc);
+        return;
+    }
     float sx, cx;
     sincosf(x, &sx, &cx);                            // full-range accurate: kd reaches ~1000 rad
     if constexpr (VARIANT == celes::kRotated) {             // the same recurrence on packed (Re, Im)

@@ -296,3 +296,23 @@ def test_bicgstab_same_solution(precond):
     assert info["converged"] and info["rel_residual"] <= 1e-4, info
     assert info["matvecs"] >= 2 * info["iterations"]
     assert rel(x.cpu().numpy(), xref) <= SOLVE_TOL
+
+
+@pytest.mark.parametrize("dr", [0.0, 4.0])
+def test_hankel_lookup_table_mode(dr):
+    """S2 of the scope table, the paper's own scheme: h_p(kd) from a lookup table with spacing dr
+    (default 1 nm as in PAPER.md:140; 4 nm still holds the tolerance with Hermite cubics) instead of the in-register
+    recurrence.  Same operator, same tolerance; C1 in full and a C3-shaped slab whose distances span many nodes."""
+    for w in (workloads.C1, workloads.scaled(workloads.C3, 1200)):
+        pos, rad, q, ctx, b = make(w, hankel="table", hankel_dr=dr)
+        recv = workloads.sample_receivers(w.N, min(w.N, 200), 306)
+        ref = orc.coupling_matvec(pos, w.k, w.lmax, b, receivers=recv)
+        assert rel(gpu_coupling(ctx, b)[recv], ref) <= MATVEC_TOL
+
+
+def test_hankel_table_needs_the_default_translation():
+    w = workloads.C1
+    pos, rad = workloads.positions(w)
+    q = fields.mie_coefficients(w.lmax, w.k, rad, workloads.N_SPHERE)
+    with pytest.raises(celes.CelesError):
+        celes.celes_setup(pos, rad, q, w.k, w.lmax, translation="direct", hankel="table")

@@ -57,6 +57,8 @@ def parse():
                     help="time celes_solve (plane wave, GMRES(30), rtol 1e-4) on the workload instead (config 5: --workload C5)")
     ap.add_argument("--precond-edge", type=float, default=0.0,
                     help="with --solve: lateral edge (nm) of the cuboids of the block-diagonal preconditioner (0 = none)")
+    ap.add_argument("--far-field", type=int, default=0, metavar="NB",
+                    help="time celes_far_field on NB x 2NB directions (Gauss-Legendre x uniform azimuth) instead")
     ap.add_argument("--hankel", default="registers", choices=["registers", "table"],
                     help="h_p(kd) in registers (default) or from the paper's lookup table (PAPER.md:130)")
     ap.add_argument("--method", default="gmres", choices=["gmres", "bicgstab"], help="with --solve")
@@ -250,6 +252,41 @@ def run_solve(args, w):
         "ms_per_matvec_incl_krylov": 1e3 * float(np.median(secs)) / max(1, info["matvecs"])}))
 
 
+def run_far_field(args, w):
+    """celes_far_field on the workload: time per call, (direction, polarisation, sphere) terms per second."""
+    import torch
+    import paper_1706_02145_b200 as celes
+    from paper_1706_02145_b200 import fields, workloads
+    torch.cuda.set_device(0)
+    pos, rad = workloads.positions(w)
+    q = fields.mie_coefficients(w.lmax, w.k, rad, workloads.N_SPHERE)
+    ctx = celes.celes_setup(pos, rad, q, w.k, w.lmax)
+    b = torch.from_numpy(workloads.gaussian_coefficients(w.N, w.nmax, w.seed_b)).cuda()
+    nb = args.far_field
+    xb, _ = np.polynomial.legendre.leggauss(nb)
+    A, B = np.meshgrid(2 * np.pi * np.arange(2 * nb) / (2 * nb), np.arccos(xb), indexing="ij")
+    al, be = A.ravel(), B.ravel()
+    g = torch.empty(al.size, 2, dtype=torch.complex64, device="cuda")
+    for _ in range(max(3, args.warmup)):
+        celes.celes_far_field(ctx, b, al, be, g)
+    times = []
+    for _ in range(max(1, args.steps)):
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        celes.celes_far_field(ctx, b, al, be, g)          # synchronises; includes the host-side direction tables
+        times.append(time.perf_counter() - t0)
+    sec = float(np.median(times))
+    terms = 2.0 * al.size * w.N
+    lane = {3: 2 * 30 * 2 + 44.0, 4: 2 * 48 * 2 + 44.0}.get(w.lmax, 0.0)      # 2 nmax FFMA2 + phase, sincos, rotation
+    sm = torch.cuda.get_device_properties(0).multi_processor_count
+    print(json.dumps({
+        "metric": "far_field_terms_per_s", "value": terms / sec, "unit": "(direction,polarisation,sphere)/s", "n_gpus": 1,
+        "steps": len(times), "ms_per_call": sec * 1e3, "higher_is_better": True, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"{w.name}: N={w.N} lmax={w.lmax}", "directions": int(al.size)},
+        "roofline": {"bound": "alu", "lane_ops_per_term": lane,
+                     "fma_pipe_utilisation_incl_host_tables": lane * terms / sec / (FP32_LANES_PER_SM * sm * 1.965e9)}}))
+
+
 def main():
     args = parse()
     from paper_1706_02145_b200 import workloads
@@ -259,6 +296,9 @@ def main():
         return
     if args.solve:
         run_solve(args, w)
+        return
+    if args.far_field > 0:
+        run_far_field(args, w)
         return
 
     import torch

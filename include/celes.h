@@ -149,6 +149,18 @@ int celes_precond_apply(celes_ctx* ctx, const void* v_dev, void* z_dev, void* cu
  * the non-empty cuboids; *n_groups (nullable) their number. */
 int celes_partition(int N, const double* pos_xyz, const double* edge_xyz, int* group_of, int* n_groups);
 
+/* Far field of the scattered field (PAPER.md:271 (A.12), 351-369 (D.1)-(D.3)): every sphere's outgoing SVWFs are turned
+ * into plane waves about its own centre with (A.12) and the contributions are added:
+ *     g_j(alpha, beta) = (1 / 2 pi) sum_i exp(-i k(alpha,beta).r_i) sum_n b^i_n B_nj(beta) exp(i m alpha),  j = 1, 2,
+ * with B_nj of (A.14) and k(alpha,beta) = k (sin beta cos alpha, sin beta sin alpha, cos beta); the radiant intensity is
+ * I_j = 2 pi^2 / (omega k mu_0) |g_j|^2 (D.3).
+ *   b_dev   device, N*nmax complex64: scattered-field coefficients (e.g. the solution of celes_solve).
+ *   alpha, beta  host, [n_dir] double: azimuthal and (real) polar angles of the directions, radians.
+ *   g_dev   device, [n_dir][2] complex64: g_1, g_2 per direction.
+ * Synchronises the stream (it frees its per-call direction tables). */
+int celes_far_field(celes_ctx* ctx, const void* b_dev, int n_dir, const double* alpha, const double* beta,
+                    void* g_dev, void* cuda_stream);
+
 /* Release the context and every device table it owns.  NULL is allowed. */
 void celes_destroy(celes_ctx* ctx);
 

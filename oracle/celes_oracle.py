@@ -4,12 +4,13 @@ FP64, CPU, plain.  Each function cites the passage of PAPER.md it restates.  The
 sum itself lives in ``celes_oracle.cpp`` (same directory) and is reached through ctypes; this
 file adds what surrounds it on the hot path: the sphere T-matrix (B.1-B.3), the system
 operator of eqs. (8)-(9), the plane-wave right-hand side (A.13-A.14), a reference solve, the
-block-diagonal preconditioner of PAPER.md:109-116 (cuboid partition, block-by-block dense solve), and
+block-diagonal preconditioner of PAPER.md:109-116 (cuboid partition, block-by-block dense solve), the far-field
+amplitudes of (A.12)/(D.1)-(D.3), and
 the SVWF / PVWF evaluators (A.2, A.4) that the pins in tests/test_oracle_pins.py use for the
 brute-force addition-theorem check.
 
 Nothing in here imports, reads or shares anything with ``paper_1706_02145_b200/``.
-Pins: see tests/test_oracle_pins.py (P1-P11, P13 of DESIGN.md).  Nothing is "parity unpinned".
+Pins: see tests/test_oracle_pins.py (P1-P11, P13, P14 of DESIGN.md).  Nothing is "parity unpinned".
 """
 from __future__ import annotations
 
@@ -395,3 +396,35 @@ def scattering_cross_section(pos, k, lmax, b) -> float:
     b = np.asarray(b, dtype=np.complex128)
     Rb = coupling_matvec(pos, k, lmax, b, kind=1) if b.shape[0] > 1 else np.zeros_like(b)
     return float((np.pi / k**2) * np.real(np.vdot(b, b + Rb)))
+
+
+# ----------------------------------------------------------------------------- far field (A.12, D.1-D.3)
+def far_field_amplitude(pos, k, lmax, b, alpha, beta) -> np.ndarray:
+    """Plane-wave amplitudes g_j(alpha, beta), j = 1, 2, of the scattered field (3) in the directions (alpha, beta)
+    (real polar angle beta: the propagating part of D.1).  Each sphere's outgoing SVWFs are turned into
+    plane waves with (A.12), about its own centre; shifting the origin to r_i multiplies
+    Phi_j(alpha, beta; r - r_i) by exp(-i k.r_i); the contributions of all spheres are added:
+
+        g_j(alpha, beta) = (1 / 2 pi) sum_i exp(-i k(alpha,beta).r_i) sum_n b^i_n B_nj(beta) exp(i m alpha).
+
+    Returns [n_dir, 2] complex128.  The radiant intensity is I_j = 2 pi^2 / (omega k mu_0) |g_j|^2 (D.3)."""
+    pos = np.atleast_2d(np.asarray(pos, dtype=np.float64))
+    b = np.asarray(b, dtype=np.complex128).reshape(pos.shape[0], nmax_of(lmax))
+    alpha = np.atleast_1d(np.asarray(alpha, dtype=np.float64))
+    beta = np.atleast_1d(np.asarray(beta, dtype=np.float64))
+    ms = np.array([m for (_, _, m) in multi_indices(lmax)])
+    g = np.zeros((alpha.shape[0], 2), dtype=np.complex128)
+    for d in range(alpha.shape[0]):
+        kvec = k * np.array([np.sin(beta[d]) * np.cos(alpha[d]), np.sin(beta[d]) * np.sin(alpha[d]), np.cos(beta[d])])
+        phase = np.exp(-1j * (pos @ kvec))
+        for j in (1, 2):
+            c = plane_wave_B(lmax, beta[d], j) * np.exp(1j * ms * alpha[d])
+            g[d, j - 1] = np.sum(phase * (b @ c)) / (2.0 * np.pi)
+    return g
+
+
+def scattered_power_cross_section(k, g, weights) -> float:
+    """(D.2) as a cross section for a unit-amplitude incident plane wave: the flux P = 2 pi^2 / (omega k mu_0)
+    sum_j int |g_j|^2 sin(beta) d(beta) d(alpha) divided by the incident intensity k / (2 omega mu_0) gives
+    (4 pi^2 / k^2) sum_j int |g_j|^2 dOmega; `weights` are the quadrature weights of the directions (dOmega)."""
+    return float(4.0 * np.pi**2 / k**2 * np.sum(np.asarray(weights)[:, None] * np.abs(g) ** 2))

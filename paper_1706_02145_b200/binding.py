@@ -26,7 +26,7 @@ CELES_MAX_HISTORY = 4096
 EXPORTS = ["celes_setup", "celes_coupling_matvec", "celes_system_matvec", "celes_coupling_matvec_host",
            "celes_system_matvec_host", "celes_solve", "celes_destroy", "celes_strerror", "celes_nmax",
            "celes_launch_config", "celes_translation_table", "celes_fp32_peak_probe", "celes_precond_setup",
-           "celes_precond_apply", "celes_partition"]
+           "celes_precond_apply", "celes_partition", "celes_far_field"]
 
 
 class CelesError(RuntimeError):
@@ -92,6 +92,8 @@ def lib() -> ctypes.CDLL:
         L.celes_precond_apply.argtypes = [p, p, p, p]
         L.celes_partition.restype = i
         L.celes_partition.argtypes = [i, p, p, p, ctypes.POINTER(i)]
+        L.celes_far_field.restype = i
+        L.celes_far_field.argtypes = [p, p, i, p, p, p, p]
         L.celes_fp32_peak_probe.restype = i
         L.celes_fp32_peak_probe.argtypes = [i, i, ctypes.POINTER(d), ctypes.POINTER(d), p]
         _LIB = L
@@ -240,6 +242,26 @@ def celes_precond_apply(ctx: Context, v, z=None, stream=None):
     if rc != CELES_OK:
         raise CelesError(rc, "celes_precond_apply")
     return z
+
+
+def celes_far_field(ctx: Context, b, alpha, beta, g=None, stream=None):
+    """g [n_dir, 2] complex64 (device): far-field amplitudes g_1, g_2 of the scattered field with coefficients b in the
+    directions (alpha, beta) (host arrays, radians); celes_far_field of include/celes.h."""
+    import torch
+    _check_vec(b, ctx, "b")
+    al = np.ascontiguousarray(alpha, dtype=np.float64).reshape(-1)
+    be = np.ascontiguousarray(beta, dtype=np.float64).reshape(-1)
+    if al.shape != be.shape or al.size < 1:
+        raise ValueError("alpha and beta: same non-zero length")
+    if g is None:
+        g = torch.empty(al.size, 2, dtype=torch.complex64, device=b.device)
+    if not (g.is_cuda and g.dtype == torch.complex64 and g.is_contiguous() and g.numel() == 2 * al.size):
+        raise ValueError("g: contiguous CUDA complex64 tensor with 2 * n_dir elements")
+    rc = lib().celes_far_field(ctx.handle, b.data_ptr(), int(al.size), al.ctypes.data, be.ctypes.data, g.data_ptr(),
+                               _stream(stream))
+    if rc != CELES_OK:
+        raise CelesError(rc, "celes_far_field")
+    return g
 
 
 def celes_partition(pos_xyz, edge_xyz):

@@ -18,6 +18,7 @@
 
 #include "../../include/celes.h"
 #include "coupling_kernel.cuh"
+#include "far_field.cuh"
 #include "krylov_kernels.cuh"
 #include "partition.h"
 #include "precond_kernels.cuh"
@@ -919,6 +920,45 @@ int celes_precond_setup(celes_ctx* ctx, const double* edge_xyz, celes_precond_in
 int celes_precond_apply(celes_ctx* ctx, const void* v_dev, void* z_dev, void* cuda_stream) {
     if (!ctx || !v_dev || !z_dev || v_dev == z_dev || !ctx->pc_ready) return CELES_EINVAL;
     return precond_apply(ctx, (const float2*)v_dev, (float2*)z_dev, (cudaStream_t)cuda_stream);
+}
+
+int celes_far_field(celes_ctx* ctx, const void* b_dev, int n_dir, const double* alpha, const double* beta, void* g_dev,
+                    void* cuda_stream) {
+    if (!ctx || !b_dev || !g_dev || n_dir < 1 || !alpha || !beta || n_dir > (1 << 29)) return CELES_EINVAL;
+    for (int d = 0; d < n_dir; ++d)
+        if (!std::isfinite(alpha[d]) || !std::isfinite(beta[d])) return CELES_EINVAL;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const int nmax = ctx->nmax, rows = 2 * n_dir, gx = (rows + celes::kFarThreads - 1) / celes::kFarThreads;
+    // split the sphere sum so that the grid has about four CTAs per SM-slot pair, at least 4 tiles per CTA
+    int splits = std::max(1, std::min((8 * ctx->sm_count + gx - 1) / gx, std::max(1, ctx->N / (4 * celes::kFarTile))));
+    const int chunk = ((ctx->N + splits - 1) / splits + celes::kFarTile - 1) / celes::kFarTile * celes::kFarTile;
+    splits = (ctx->N + chunk - 1) / chunk;
+    double *d_ang = nullptr, *d_dir = nullptr;
+    float2 *d_coef = nullptr, *d_part = nullptr;
+    int rc = CELES_OK;
+    if (cudaMalloc(&d_ang, sizeof(double) * 2 * (size_t)n_dir) != cudaSuccess ||
+        cudaMalloc(&d_dir, sizeof(double) * 3 * (size_t)n_dir) != cudaSuccess ||
+        cudaMalloc(&d_coef, sizeof(float2) * (size_t)rows * nmax) != cudaSuccess ||
+        cudaMalloc(&d_part, sizeof(float2) * (size_t)rows * splits) != cudaSuccess) rc = CELES_ENOMEM;
+    if (!rc && (cudaMemcpyAsync(d_ang, alpha, sizeof(double) * n_dir, cudaMemcpyHostToDevice, s) != cudaSuccess ||
+                cudaMemcpyAsync(d_ang + n_dir, beta, sizeof(double) * n_dir, cudaMemcpyHostToDevice, s) != cudaSuccess)) rc = CELES_ECUDA;
+    if (!rc) {
+        celes::far_field_coefficients_kernel<<<(n_dir + 127) / 128, 128, 0, s>>>(ctx->lmax, n_dir, d_ang, d_ang + n_dir, d_coef, d_dir);
+        const float2* b = (const float2*)b_dev;
+        dim3 grid(gx, splits);
+        switch (ctx->lmax) {
+            case 1: celes::far_field_kernel<6><<<grid, celes::kFarThreads, 0, s>>>(ctx->N, chunk, rows, ctx->kpos, b, d_coef, d_dir, d_part); break;
+            case 2: celes::far_field_kernel<16><<<grid, celes::kFarThreads, 0, s>>>(ctx->N, chunk, rows, ctx->kpos, b, d_coef, d_dir, d_part); break;
+            case 3: celes::far_field_kernel<30><<<grid, celes::kFarThreads, 0, s>>>(ctx->N, chunk, rows, ctx->kpos, b, d_coef, d_dir, d_part); break;
+            case 4: celes::far_field_kernel<48><<<grid, celes::kFarThreads, 0, s>>>(ctx->N, chunk, rows, ctx->kpos, b, d_coef, d_dir, d_part); break;
+            default: rc = CELES_EINVAL;
+        }
+        if (!rc) celes::far_field_reduce_kernel<<<(rows + 255) / 256, 256, 0, s>>>(rows, splits, d_part, (float2*)g_dev);
+        if (!rc && cudaGetLastError() != cudaSuccess) rc = CELES_ECUDA;
+    }
+    if (cudaStreamSynchronize(s) != cudaSuccess && !rc) rc = CELES_ECUDA;
+    cudaFree(d_ang); cudaFree(d_dir); cudaFree(d_coef); cudaFree(d_part);
+    return rc;
 }
 
 void celes_destroy(celes_ctx* ctx) { free_ctx(ctx); }

@@ -316,3 +316,41 @@ def test_hankel_table_needs_the_default_translation():
     q = fields.mie_coefficients(w.lmax, w.k, rad, workloads.N_SPHERE)
     with pytest.raises(celes.CelesError):
         celes.celes_setup(pos, rad, q, w.k, w.lmax, translation="direct", hankel="table")
+
+
+@pytest.mark.parametrize("lmax", [1, 2, 3, 4])
+def test_far_field_matches_oracle(lmax):
+    """celes_far_field (A.12, D.1-D.3) against the oracle, direction by direction, on random coefficients: forward,
+    backward, grazing and generic directions, every lmax; FP32 sums over N spheres with FP64 phases."""
+    import dataclasses
+    w = dataclasses.replace(workloads.scaled(workloads.C3, 700), lmax=lmax)
+    pos, rad, q, ctx, b = make(w)
+    rng = np.random.default_rng(406)
+    alpha = np.concatenate([[0.0, 0.0, 1.0, 2.5], rng.uniform(0, 2 * np.pi, 60)])
+    beta = np.concatenate([[0.0, np.pi, np.pi / 2, 1e-3], np.arccos(rng.uniform(-1, 1, 60))])
+    g = celes.celes_far_field(ctx, torch.from_numpy(b).cuda(), alpha, beta).cpu().numpy()
+    ref = orc.far_field_amplitude(pos, w.k, w.lmax, b, alpha, beta)
+    assert g.shape == (64, 2)
+    assert rel(g, ref) <= MATVEC_TOL
+    assert np.max(np.abs(g - ref)) <= 1e-3 * np.max(np.abs(ref))
+
+
+def test_far_field_of_a_solution_carries_the_scattered_power():
+    """Energy check available without the Gaussian beam (PAPER.md:146 checks R + T): the far-field flux of the GPU
+    solution, integrated over all directions by Gauss-Legendre x uniform azimuth, equals the extinction of the
+    plane wave (optical theorem, lossless spheres) and the oracle's C_sca."""
+    w = workloads.scaled(workloads.C2, 120)
+    pos, rad, q, ctx, _ = make(w)
+    a_in = orc.plane_wave_a_in(pos, w.k, w.lmax)
+    x = torch.zeros(w.N, w.nmax, dtype=torch.complex64, device="cuda")
+    info = celes.celes_solve(ctx, torch.from_numpy(a_in.astype(np.complex64)).cuda(), x, rtol=1e-5)
+    assert info["converged"]
+    xb, wb = np.polynomial.legendre.leggauss(64)
+    na = 128
+    A, B = np.meshgrid(2 * np.pi * np.arange(na) / na, np.arccos(xb), indexing="ij")
+    W = np.broadcast_to(wb[None, :] * 2 * np.pi / na, A.shape).ravel()
+    g = celes.celes_far_field(ctx, x, A.ravel(), B.ravel()).cpu().numpy().astype(np.complex128)
+    csca_ff = orc.scattered_power_cross_section(w.k, g, W)
+    xg = x.cpu().numpy().astype(np.complex128)
+    assert abs(csca_ff - orc.scattering_cross_section(pos, w.k, w.lmax, xg)) / csca_ff <= 1e-3
+    assert abs(csca_ff - orc.extinction_cross_section(w.k, a_in, xg)) / csca_ff <= 2e-3

@@ -378,3 +378,34 @@ def test_p13_preconditioner_limits_and_partition_brute_force():
         rows = (idx[:, None] * n + np.arange(n)[None, :]).reshape(-1)
         assert _rel(Mf[np.ix_(rows, rows)] @ zf[idx].reshape(-1), v[idx].reshape(-1)) < 1e-11
     assert _rel(Mf @ zf.reshape(-1), v.reshape(-1)) < 1e-2      # coupling ~ 1/(k d) across 400 um
+
+
+# --------------------------------------------------------------------------- P14 far field (A.12, D.1-D.3)
+def test_p14_far_field_power_equals_scattering_cross_section(golden):
+    """The flux of the plane-wave amplitudes g_j (A.12 about every sphere, D.2) over the full sphere of directions
+    equals C_sca of P8 (golden value, PAPER-derived; and the oracle's regular-translation formula): fixes the 1/2pi of
+    (A.12), the prefactor of (D.2)-(D.3), the sign of the origin-shift phase and the roles of B_n1, B_n2.  A rigid
+    shift of the cluster multiplies g by a pure phase; a single sphere with one coefficient gives |B_nj| / 2 pi."""
+    g8 = golden("p8_optical_theorem.txt")
+    q = o.mie_q(3, K, [100.0] * 3, 1.52)
+    a_in = o.plane_wave_a_in(POS3, K, 3)
+    b = o.solve_dense(POS3, K, 3, q, a_in)
+    xb, wb = np.polynomial.legendre.leggauss(40)
+    na = 80
+    A, B = np.meshgrid(2 * np.pi * np.arange(na) / na, np.arccos(xb), indexing="ij")
+    W = np.broadcast_to(wb[None, :] * 2 * np.pi / na, A.shape)
+    g = o.far_field_amplitude(POS3, K, 3, b, A.ravel(), B.ravel())
+    csca = o.scattered_power_cross_section(K, g, W.ravel())
+    assert csca == pytest.approx(g8["C_sca_nm2"][0], rel=1e-9)
+    assert csca == pytest.approx(o.scattering_cross_section(POS3, K, 3, b), rel=1e-9)
+    shift = np.array([310.0, -120.0, 75.0])
+    gs = o.far_field_amplitude(POS3 + shift, K, 3, b, A.ravel()[:50], B.ravel()[:50])
+    kv = K * np.stack([np.sin(B.ravel()[:50]) * np.cos(A.ravel()[:50]), np.sin(B.ravel()[:50]) * np.sin(A.ravel()[:50]),
+                       np.cos(B.ravel()[:50])], axis=1)
+    assert np.allclose(gs, g[:50] * np.exp(-1j * (kv @ shift))[:, None], rtol=1e-12, atol=1e-15)
+    e = np.zeros((1, o.nmax_of(3)), dtype=np.complex128)
+    n = o.nindex(3, 2, 2, -1)
+    e[0, n] = 1.0
+    g1 = o.far_field_amplitude(np.zeros((1, 3)), K, 3, e, [0.7], [1.1])
+    for j in (1, 2):
+        assert g1[0, j - 1] == pytest.approx(o.plane_wave_B(3, 1.1, j)[n] * np.exp(-1j * 0.7) / (2 * np.pi), rel=1e-13)

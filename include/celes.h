@@ -161,6 +161,21 @@ int celes_partition(int N, const double* pos_xyz, const double* edge_xyz, int* g
 int celes_far_field(celes_ctx* ctx, const void* b_dev, int n_dir, const double* alpha, const double* beta,
                     void* g_dev, void* cuda_stream);
 
+/* Gaussian beam of Appendix C: waist w centred at r_G, propagating along +z, field at the waist
+ * E_0 (-sin alpha_G e_x + cos alpha_G e_y) exp(-((x-x_G)^2 + (y-y_G)^2)/w^2) (C.1). */
+typedef struct celes_beam {
+    double waist;          /* w > 0, length unit U */
+    double center[3];      /* r_G */
+    double alpha_G;        /* polarisation angle, radians */
+    double E0_re, E0_im;   /* complex amplitude E_0 */
+    int n_beta;            /* Gauss-Legendre nodes of the polar-angle integral over [0, pi/2]; 0 = default 400 */
+} celes_beam;
+
+/* Initial-field coefficients a_in of the beam about every sphere centre, (C.8) with the analytic azimuthal integral
+ * (C.7), evaluated on the device in FP64 and rounded once.  a_in_dev: device, N*nmax complex64 (the
+ * input of celes_solve).  Synchronises the stream. */
+int celes_gaussian_beam(celes_ctx* ctx, const celes_beam* beam, void* a_in_dev, void* cuda_stream);
+
 /* Release the context and every device table it owns.  NULL is allowed. */
 void celes_destroy(celes_ctx* ctx);
 

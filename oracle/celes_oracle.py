@@ -5,12 +5,12 @@ sum itself lives in ``celes_oracle.cpp`` (same directory) and is reached through
 file adds what surrounds it on the hot path: the sphere T-matrix (B.1-B.3), the system
 operator of eqs. (8)-(9), the plane-wave right-hand side (A.13-A.14), a reference solve, the
 block-diagonal preconditioner of PAPER.md:109-116 (cuboid partition, block-by-block dense solve), the far-field
-amplitudes of (A.12)/(D.1)-(D.3), and
+amplitudes of (A.12)/(D.1)-(D.3), the Gaussian beam of Appendix C, and
 the SVWF / PVWF evaluators (A.2, A.4) that the pins in tests/test_oracle_pins.py use for the
 brute-force addition-theorem check.
 
 Nothing in here imports, reads or shares anything with ``paper_1706_02145_b200/``.
-Pins: see tests/test_oracle_pins.py (P1-P11, P13, P14 of DESIGN.md).  Nothing is "parity unpinned".
+Pins: see tests/test_oracle_pins.py (P1-P11, P13-P15 of DESIGN.md).  Nothing is "parity unpinned".
 """
 from __future__ import annotations
 
@@ -428,3 +428,73 @@ def scattered_power_cross_section(k, g, weights) -> float:
     sum_j int |g_j|^2 sin(beta) d(beta) d(alpha) divided by the incident intensity k / (2 omega mu_0) gives
     (4 pi^2 / k^2) sum_j int |g_j|^2 dOmega; `weights` are the quadrature weights of the directions (dOmega)."""
     return float(4.0 * np.pi**2 / k**2 * np.sum(np.asarray(weights)[:, None] * np.abs(g) ** 2))
+
+
+# ----------------------------------------------------------------------------- Gaussian beam (Appendix C, D.4-D.5)
+def _beam_polarisation(j, alpha, alpha_G):
+    """(C.3)-(C.4): e^{i(a-aG)} (d_j1 - i d_j2)/2 + e^{-i(a-aG)} (d_j1 + i d_j2)/2."""
+    d1, d2 = (1.0, 0.0) if j == 1 else (0.0, 1.0)
+    return np.exp(1j * (alpha - alpha_G)) * (d1 - 1j * d2) / 2 + np.exp(-1j * (alpha - alpha_G)) * (d1 + 1j * d2) / 2
+
+
+def gaussian_beam_a_in(pos, k, lmax, w, r_G, alpha_G=0.0, E0=1.0, n_beta=400) -> np.ndarray:
+    """Initial-field coefficients of the Gaussian beam of Appendix C (waist w at r_G, propagating along +z,
+    polarisation angle alpha_G), (C.8), with the alpha-integral I_jn(beta) of (C.7)
+    (readings R20: I_j of C.8 is I_jn, B_jn^dagger of C.6 is B_nj^dagger).  The beta-integral over [0, pi/2] is
+    evaluated with n_beta Gauss-Legendre nodes.  Returns [N, nmax] complex128."""
+    from scipy.special import jv
+    pos = np.atleast_2d(np.asarray(pos, dtype=np.float64))
+    rel = pos - np.asarray(r_G, dtype=np.float64)[None, :]
+    rho, phi, z = np.hypot(rel[:, 0], rel[:, 1]), np.arctan2(rel[:, 1], rel[:, 0]), rel[:, 2]
+    x, wq = np.polynomial.legendre.leggauss(n_beta)
+    beta, wq = (x + 1.0) * np.pi / 4.0, wq * np.pi / 4.0
+    idx = multi_indices(lmax)
+    a = np.zeros((pos.shape[0], nmax_of(lmax)), dtype=np.complex128)
+    for q in range(n_beta):
+        sb, cb = np.sin(beta[q]), np.cos(beta[q])
+        common = wq[q] * sb * cb * np.exp(-w * w * k * k * sb * sb / 4.0) * np.exp(1j * k * z * cb)      # [N]
+        for j in (1, 2):
+            Bd = plane_wave_B(lmax, beta[q], j, dagger=True)
+            d1, d2 = (1.0, 0.0) if j == 1 else (0.0, 1.0)
+            for n, (tau, l, m) in enumerate(idx):
+                I = (2 * np.pi * np.exp(-1j * alpha_G) * 1j ** abs(m - 1) * np.exp(-1j * (m - 1) * phi)
+                     * jv(abs(m - 1), k * rho * sb) * (d1 - 1j * d2) / 2
+                     + 2 * np.pi * np.exp(1j * alpha_G) * 1j ** abs(m + 1) * np.exp(-1j * (m + 1) * phi)
+                     * jv(abs(m + 1), k * rho * sb) * (d1 + 1j * d2) / 2)
+                a[:, n] += common * Bd[n] * I
+    return E0 * k * k * w * w / np.pi * a
+
+
+def gaussian_beam_a_in_brute_force(pos, k, lmax, w, r_G, alpha_G=0.0, E0=1.0, n_beta=200, n_alpha=256) -> np.ndarray:
+    """The same coefficients straight from the angular spectrum (C.4), with the exact phase
+    e^{i k.(r_i - r_G)} (the product of the two exponentials of (C.5), reading R20) and (A.13) for every plane wave;
+    both integrals by quadrature (uniform in alpha, Gauss-Legendre in beta).  Small N only."""
+    pos = np.atleast_2d(np.asarray(pos, dtype=np.float64))
+    rel = pos - np.asarray(r_G, dtype=np.float64)[None, :]
+    x, wq = np.polynomial.legendre.leggauss(n_beta)
+    beta, wq = (x + 1.0) * np.pi / 4.0, wq * np.pi / 4.0
+    alpha = 2 * np.pi * np.arange(n_alpha) / n_alpha
+    ms = np.array([m for (_, _, m) in multi_indices(lmax)])
+    a = np.zeros((pos.shape[0], nmax_of(lmax)), dtype=np.complex128)
+    for q in range(n_beta):
+        sb, cb = np.sin(beta[q]), np.cos(beta[q])
+        amp = wq[q] * sb * cb * np.exp(-w * w * k * k * sb * sb / 4.0) * (2 * np.pi / n_alpha)
+        kvec = k * np.stack([sb * np.cos(alpha), sb * np.sin(alpha), np.full_like(alpha, cb)], axis=1)      # [na, 3]
+        phase = np.exp(1j * (rel @ kvec.T))                                                                 # [N, na]
+        for j in (1, 2):
+            Bd = plane_wave_B(lmax, beta[q], j, dagger=True)
+            pol = _beam_polarisation(j, alpha, alpha_G)                                                     # [na]
+            # Phi_j(alpha, beta; r - r_i) = 4 sum_n e^{-i m alpha} B^dagger_nj Psi_n^(1)(r - r_i)   (A.13)
+            a += amp * (phase * pol[None, :]) @ (4.0 * np.exp(-1j * np.outer(alpha, ms)) * Bd[None, :])
+    return E0 * k * k * w * w / (4 * np.pi) * a
+
+
+def gaussian_beam_g(k, w, r_G, alpha, beta, alpha_G=0.0, E0=1.0) -> np.ndarray:
+    """Plane-wave amplitudes of the beam, (D.4), for polarisation angle alpha_G (D.4 prints alpha_G = 0):
+    g_j = E0 k^2 w^2 / (4 pi) cos(beta) exp(-w^2 k^2 sin^2(beta) / 4) (d_j1 cos(a - aG) + d_j2 sin(a - aG)) e^{-i k.r_G};
+    zero for beta > pi/2 (the beam only contains waves travelling towards +z).  [n_dir, 2]."""
+    alpha = np.atleast_1d(np.asarray(alpha, dtype=np.float64)); beta = np.atleast_1d(np.asarray(beta, dtype=np.float64))
+    kvec = k * np.stack([np.sin(beta) * np.cos(alpha), np.sin(beta) * np.sin(alpha), np.cos(beta)], axis=1)
+    amp = E0 * k * k * w * w / (4 * np.pi) * np.cos(beta) * np.exp(-w * w * k * k * np.sin(beta) ** 2 / 4.0)
+    amp = np.where(beta <= np.pi / 2, amp, 0.0) * np.exp(-1j * (kvec @ np.asarray(r_G, dtype=np.float64)))
+    return np.stack([amp * np.cos(alpha - alpha_G), amp * np.sin(alpha - alpha_G)], axis=1)

@@ -26,7 +26,7 @@ CELES_MAX_HISTORY = 4096
 EXPORTS = ["celes_setup", "celes_coupling_matvec", "celes_system_matvec", "celes_coupling_matvec_host",
            "celes_system_matvec_host", "celes_solve", "celes_destroy", "celes_strerror", "celes_nmax",
            "celes_launch_config", "celes_translation_table", "celes_fp32_peak_probe", "celes_precond_setup",
-           "celes_precond_apply", "celes_partition", "celes_far_field"]
+           "celes_precond_apply", "celes_partition", "celes_far_field", "celes_gaussian_beam"]
 
 
 class CelesError(RuntimeError):
@@ -43,6 +43,11 @@ class celes_options(ctypes.Structure):
 class celes_solve_opts(ctypes.Structure):
     _fields_ = [("method", ctypes.c_int), ("restart", ctypes.c_int), ("rtol", ctypes.c_double),
                 ("max_iters", ctypes.c_int), ("precond", ctypes.c_int)]
+
+
+class celes_beam(ctypes.Structure):
+    _fields_ = [("waist", ctypes.c_double), ("center", ctypes.c_double * 3), ("alpha_G", ctypes.c_double),
+                ("E0_re", ctypes.c_double), ("E0_im", ctypes.c_double), ("n_beta", ctypes.c_int)]
 
 
 class celes_precond_info(ctypes.Structure):
@@ -92,6 +97,8 @@ def lib() -> ctypes.CDLL:
         L.celes_precond_apply.argtypes = [p, p, p, p]
         L.celes_partition.restype = i
         L.celes_partition.argtypes = [i, p, p, p, ctypes.POINTER(i)]
+        L.celes_gaussian_beam.restype = i
+        L.celes_gaussian_beam.argtypes = [p, ctypes.POINTER(celes_beam), p, p]
         L.celes_far_field.restype = i
         L.celes_far_field.argtypes = [p, p, i, p, p, p, p]
         L.celes_fp32_peak_probe.restype = i
@@ -242,6 +249,22 @@ def celes_precond_apply(ctx: Context, v, z=None, stream=None):
     if rc != CELES_OK:
         raise CelesError(rc, "celes_precond_apply")
     return z
+
+
+def celes_gaussian_beam(ctx: Context, waist: float, center, alpha_G: float = 0.0, E0: complex = 1.0, n_beta: int = 0,
+                        a_in=None, stream=None):
+    """a_in [N, nmax] complex64 (device) of the Gaussian beam of Appendix C; celes_gaussian_beam of include/celes.h."""
+    import torch
+    if a_in is None:
+        a_in = torch.empty(ctx.N, ctx.nmax, dtype=torch.complex64, device="cuda")
+    _check_vec(a_in, ctx, "a_in")
+    c = np.asarray(center, dtype=np.float64).reshape(3)
+    beam = celes_beam(float(waist), (ctypes.c_double * 3)(*c), float(alpha_G), float(complex(E0).real),
+                      float(complex(E0).imag), int(n_beta))
+    rc = lib().celes_gaussian_beam(ctx.handle, ctypes.byref(beam), a_in.data_ptr(), _stream(stream))
+    if rc != CELES_OK:
+        raise CelesError(rc, "celes_gaussian_beam")
+    return a_in
 
 
 def celes_far_field(ctx: Context, b, alpha, beta, g=None, stream=None):

@@ -19,6 +19,7 @@
 #include "../../include/celes.h"
 #include "coupling_kernel.cuh"
 #include "far_field.cuh"
+#include "gaussian_beam.cuh"
 #include "krylov_kernels.cuh"
 #include "partition.h"
 #include "precond_kernels.cuh"
@@ -958,6 +959,38 @@ int celes_far_field(celes_ctx* ctx, const void* b_dev, int n_dir, const double* 
     }
     if (cudaStreamSynchronize(s) != cudaSuccess && !rc) rc = CELES_ECUDA;
     cudaFree(d_ang); cudaFree(d_dir); cudaFree(d_coef); cudaFree(d_part);
+    return rc;
+}
+
+int celes_gaussian_beam(celes_ctx* ctx, const celes_beam* beam, void* a_in_dev, void* cuda_stream) {
+    if (!ctx || !beam || !a_in_dev) return CELES_EINVAL;
+    const int n_beta = beam->n_beta > 0 ? beam->n_beta : 400;
+    if (!(beam->waist > 0.0) || !std::isfinite(beam->waist) || n_beta > 100000) return CELES_EINVAL;
+    for (int a = 0; a < 3; ++a) if (!std::isfinite(beam->center[a])) return CELES_EINVAL;
+    if (!std::isfinite(beam->alpha_G) || !std::isfinite(beam->E0_re) || !std::isfinite(beam->E0_im)) return CELES_EINVAL;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    std::vector<double> sb, cb;
+    std::vector<double2> cminus, cplus;
+    celes::gaussian_beam_tables(ctx->lmax, n_beta, ctx->k, beam->waist, sb, cb, cminus, cplus);
+    double *d_sb = nullptr, *d_cb = nullptr;
+    double2 *d_cm = nullptr, *d_cp = nullptr;
+    int rc = CELES_OK;
+    if (cudaMalloc(&d_sb, sizeof(double) * n_beta) != cudaSuccess || cudaMalloc(&d_cb, sizeof(double) * n_beta) != cudaSuccess ||
+        cudaMalloc(&d_cm, sizeof(double2) * cminus.size()) != cudaSuccess ||
+        cudaMalloc(&d_cp, sizeof(double2) * cplus.size()) != cudaSuccess) rc = CELES_ENOMEM;
+    if (!rc && (cudaMemcpyAsync(d_sb, sb.data(), sizeof(double) * n_beta, cudaMemcpyHostToDevice, s) != cudaSuccess ||
+                cudaMemcpyAsync(d_cb, cb.data(), sizeof(double) * n_beta, cudaMemcpyHostToDevice, s) != cudaSuccess ||
+                cudaMemcpyAsync(d_cm, cminus.data(), sizeof(double2) * cminus.size(), cudaMemcpyHostToDevice, s) != cudaSuccess ||
+                cudaMemcpyAsync(d_cp, cplus.data(), sizeof(double2) * cplus.size(), cudaMemcpyHostToDevice, s) != cudaSuccess)) rc = CELES_ECUDA;
+    if (!rc) {
+        const long long total = (long long)ctx->N * ctx->nmax;
+        celes::gaussian_beam_kernel<<<(unsigned)((total + 127) / 128), 128, 0, s>>>(
+            ctx->N, ctx->lmax, n_beta, ctx->kpos, ctx->k * beam->center[0], ctx->k * beam->center[1], ctx->k * beam->center[2],
+            beam->alpha_G, make_double2(beam->E0_re, beam->E0_im), d_sb, d_cb, d_cm, d_cp, (float2*)a_in_dev);
+        if (cudaGetLastError() != cudaSuccess) rc = CELES_ECUDA;
+    }
+    if (cudaStreamSynchronize(s) != cudaSuccess && !rc) rc = CELES_ECUDA;
+    cudaFree(d_sb); cudaFree(d_cb); cudaFree(d_cm); cudaFree(d_cp);
     return rc;
 }
 

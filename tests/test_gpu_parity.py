@@ -354,3 +354,43 @@ def test_far_field_of_a_solution_carries_the_scattered_power():
     xg = x.cpu().numpy().astype(np.complex128)
     assert abs(csca_ff - orc.scattering_cross_section(pos, w.k, w.lmax, xg)) / csca_ff <= 1e-3
     assert abs(csca_ff - orc.extinction_cross_section(w.k, a_in, xg)) / csca_ff <= 2e-3
+
+
+@pytest.mark.parametrize("lmax", [1, 3, 4])
+def test_gaussian_beam_coefficients_match_oracle(lmax):
+    """celes_gaussian_beam ((C.7)-(C.8), FP64 on the device, rounded once) against the oracle's literal evaluation."""
+    import dataclasses
+    w = dataclasses.replace(workloads.scaled(workloads.C3, 300), lmax=lmax)
+    pos, rad, q, ctx, _ = make(w)
+    waist, rG, aG, E0 = 1500.0, np.array([200.0, -100.0, 150.0]), 0.3, 0.8 - 0.5j
+    a = celes.celes_gaussian_beam(ctx, waist, rG, aG, E0, n_beta=300).cpu().numpy()
+    ref = orc.gaussian_beam_a_in(pos, w.k, w.lmax, waist, rG, aG, E0, n_beta=300)
+    assert rel(a, ref) <= 1e-6
+
+
+def test_gaussian_beam_energy_balance_R_plus_T():
+    """The paper's end-to-end check (R + T = 1 within 1e-3 for lossless spheres), on a small slab:
+    Gaussian beam (Appendix C) -> celes_solve -> celes_far_field -> power flux (D.2): reflected = flux of the scattered
+    field into z < 0, transmitted = flux of beam + scattered field into z > 0, both relative to the beam power (D.5)."""
+    w = workloads.scaled(workloads.C3, 600)
+    pos, rad, q, ctx, _ = make(w)
+    waist, rG = 1200.0, np.array([0.0, 0.0, 0.5 * (pos[:, 2].min() + pos[:, 2].max())])
+    a_in = celes.celes_gaussian_beam(ctx, waist, rG)
+    x = torch.zeros(w.N, w.nmax, dtype=torch.complex64, device="cuda")
+    info = celes.celes_solve(ctx, a_in, x, rtol=1e-5, max_iters=2000)
+    assert info["converged"]
+    xb, wb = np.polynomial.legendre.leggauss(160)
+    na = 192
+    P = {}
+    for name, lo in (("T", 0.0), ("R", np.pi / 2)):
+        beta, wbeta = lo + (xb + 1.0) * np.pi / 4.0, wb * np.pi / 4.0
+        A, B = np.meshgrid(2 * np.pi * np.arange(na) / na, beta, indexing="ij")
+        W = np.broadcast_to((wbeta * np.sin(beta))[None, :] * 2 * np.pi / na, A.shape).ravel()
+        g = celes.celes_far_field(ctx, x, A.ravel(), B.ravel()).cpu().numpy().astype(np.complex128)
+        g_in = orc.gaussian_beam_g(w.k, waist, rG, A.ravel(), B.ravel())
+        P[name] = np.sum(W[:, None] * np.abs(g + g_in) ** 2)
+        if name == "T":
+            P["in"] = np.sum(W[:, None] * np.abs(g_in) ** 2)
+    R, T = P["R"] / P["in"], P["T"] / P["in"]
+    assert 0.0 < R < 1.0 and 0.0 < T < 1.0
+    assert abs(R + T - 1.0) <= 3e-3, (R, T)

@@ -409,3 +409,33 @@ def test_p14_far_field_power_equals_scattering_cross_section(golden):
     g1 = o.far_field_amplitude(np.zeros((1, 3)), K, 3, e, [0.7], [1.1])
     for j in (1, 2):
         assert g1[0, j - 1] == pytest.approx(o.plane_wave_B(3, 1.1, j)[n] * np.exp(-1j * 0.7) / (2 * np.pi), rel=1e-13)
+
+
+# --------------------------------------------------------------------------- P15 Gaussian beam (Appendix C)
+def test_p15_gaussian_beam_coefficients():
+    """(C.8) with the analytic azimuthal integral (C.7) against the angular spectrum (C.4) integrated by brute force
+    with the exact phase e^{ik.(r_i - r_G)} (fixes reading R20 of the garbled (C.5), the Bessel identity, the orders
+    |m -+ 1| and the factor k^2 w^2 / pi); the field rebuilt from the coefficients near the waist against the Gaussian
+    profile of (C.1) (fixes k^2 w^2 / 4 pi and the polarisation vector; paraxial, so to ~1/(kw)^2); and the beam power:
+    the flux of g of (D.4) equals (D.5)."""
+    pos = np.array([[0.0, 0.0, 0.0], [230.0, 40.0, -60.0], [-800.0, 1250.0, 150.0], [1500.0, -300.0, -200.0]])
+    w, rG, aG = 2000.0, np.array([100.0, -50.0, 30.0]), 0.4
+    a = o.gaussian_beam_a_in(pos, K, 3, w, rG, aG, n_beta=300)
+    a_bf = o.gaussian_beam_a_in_brute_force(pos, K, 3, w, rG, aG)
+    assert np.max(np.abs(a - a_bf)) <= 1e-12 * np.max(np.abs(a))
+    for r in (np.array([[30.0, -20.0, 30.0]]), np.array([[-15.0, 25.0, 30.0]])):
+        E = np.zeros(3, dtype=np.complex128)
+        for n, (tau, l, m) in enumerate(o.multi_indices(3)):
+            E += a[0, n] * o.svwf(1, tau, l, m, K, r - pos[0:1])[0]
+        rho2 = np.sum((r[0, :2] - rG[:2]) ** 2)
+        ref = np.exp(-rho2 / w**2) * np.array([-np.sin(aG), np.cos(aG), 0.0])
+        assert np.max(np.abs(E - ref)) <= 6e-3
+    xb, wb = np.polynomial.legendre.leggauss(400)
+    beta, wbeta = (xb + 1.0) * np.pi / 4.0, wb * np.pi / 4.0
+    na = 16
+    A, B = np.meshgrid(2 * np.pi * np.arange(na) / na, beta, indexing="ij")
+    W = np.broadcast_to((wbeta * np.sin(beta))[None, :] * 2 * np.pi / na, A.shape)
+    g = o.gaussian_beam_g(K, w, rG, A.ravel(), B.ravel(), aG)
+    flux = np.sum(W.ravel()[:, None] * np.abs(g) ** 2)                      # int sum_j |g_j|^2 sin(beta) d(beta) d(alpha)
+    d5 = K**4 * w**4 / (8 * np.pi) * np.sum(wbeta * np.sin(beta) * np.cos(beta) ** 2 * np.exp(-w * w * K * K * np.sin(beta) ** 2 / 2))
+    assert flux == pytest.approx(d5, rel=1e-12)                             # (D.5) / (2 pi^2 / (omega k mu_0))

@@ -405,6 +405,27 @@ def main():
                          "lane_rate_vs_3_operand_probe": lane_rate / (0.5 * probe[3]),
                          "lane_rate_vs_shared_multiplicand_probe": lane_rate / (0.5 * probe[4])},
         }
+        if w.name == "C4" and world == 1:
+            # BASELINE.json's metric names N = 1e4 as well: the same measurement on C3, reported beside the headline
+            w3 = workloads.CONFIGS["C3"]
+            pos3, rad3 = workloads.positions(w3)
+            ctx3 = celes.celes_setup(pos3, rad3, fields.mie_coefficients(w3.lmax, w3.k, rad3, workloads.N_SPHERE), w3.k,
+                                     w3.lmax, translation=args.translation, hankel=args.hankel)
+            b3 = torch.from_numpy(workloads.gaussian_coefficients(w3.N, w3.nmax, w3.seed_b)).cuda()
+            y3 = torch.empty_like(b3)
+            for _ in range(max(3, args.warmup)):
+                celes.celes_coupling_matvec(ctx3, b3, y3)
+            ev3 = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(10)]
+            for a3, c3 in ev3:
+                flush.zero_()
+                a3.record(stream)
+                celes.celes_coupling_matvec(ctx3, b3, y3)
+                c3.record(stream)
+            torch.cuda.synchronize()
+            ms3 = float(np.median([a3.elapsed_time(c3) for a3, c3 in ev3]))
+            line["also"] = {"workload": f"C3: N={w3.N} lmax={w3.lmax} (same recipe, 20 um slab)", "ms_per_step": ms3,
+                            "value": w3.N * (w3.N - 1) / (ms3 * 1e-3), "unit": UNIT, "steps": 10,
+                            "launch": celes.celes_launch_config(ctx3)}
         if not args.no_cpu_baseline and world == 1:
             rate, cores, n_recv, dt = oracle_sample_rate(w, pos, b_host, args.cpu_seconds)
             line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",

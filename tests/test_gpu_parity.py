@@ -394,3 +394,21 @@ def test_gaussian_beam_energy_balance_R_plus_T():
     R, T = P["R"] / P["in"], P["T"] / P["in"]
     assert 0.0 < R < 1.0 and 0.0 < T < 1.0
     assert abs(R + T - 1.0) <= 3e-3, (R, T)
+
+
+def test_solve_warm_start_from_x0():
+    """celes_solve reads x0 from x ('custom initial condition' from a sub-system): starting at the
+    converged solution needs no iteration; starting from a rough solution needs fewer than starting from zero."""
+    w = workloads.scaled(workloads.C3, 500)
+    pos, rad, q, ctx, _ = make(w)
+    a_dev = torch.from_numpy(orc.plane_wave_a_in(pos, w.k, w.lmax).astype(np.complex64)).cuda()
+    x = torch.zeros(w.N, w.nmax, dtype=torch.complex64, device="cuda")
+    cold = celes.celes_solve(ctx, a_dev, x, rtol=1e-5)
+    assert cold["converged"] and cold["iterations"] > 5
+    again = celes.celes_solve(ctx, a_dev, x, rtol=1e-4)
+    assert again["converged"] and again["iterations"] == 0 and again["matvecs"] == 1
+    rough = torch.zeros_like(x)
+    celes.celes_solve(ctx, a_dev, rough, rtol=1e-2)
+    warm = celes.celes_solve(ctx, a_dev, rough, rtol=1e-5)
+    assert warm["converged"] and warm["iterations"] < cold["iterations"]
+    assert rel(rough.cpu().numpy(), x.cpu().numpy()) <= 1e-3

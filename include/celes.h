@@ -176,6 +176,16 @@ typedef struct celes_beam {
  * input of celes_solve).  Synchronises the stream. */
 int celes_gaussian_beam(celes_ctx* ctx, const celes_beam* beam, void* a_in_dev, void* cuda_stream);
 
+/* Scattered electric field at n_pts points, eq. (3) with the explicit outgoing SVWFs (A.2):
+ *     E_scat(r) = sum_i sum_n b^i_n Psi^(3)_n(r - r_i)          (the near-field maps of Figs. 2 and 6).
+ *   b_dev    device, N*nmax complex64.
+ *   pts_xyz  host, [n_pts][3] double, unit U.  The expansion of sphere i holds for |r - r_i| > R_i only: points inside
+ *            a sphere get the (meaningless) analytic continuation, not the internal field.
+ *   e_dev    device, [n_pts][3] complex64: Cartesian components (x, y, z).
+ * Synchronises the stream. */
+int celes_scattered_field(celes_ctx* ctx, const void* b_dev, int n_pts, const double* pts_xyz, void* e_dev,
+                          void* cuda_stream);
+
 /* Release the context and every device table it owns.  NULL is allowed. */
 void celes_destroy(celes_ctx* ctx);
 

@@ -10,7 +10,7 @@ the SVWF / PVWF evaluators (A.2, A.4) that the pins in tests/test_oracle_pins.py
 brute-force addition-theorem check.
 
 Nothing in here imports, reads or shares anything with ``paper_1706_02145_b200/``.
-Pins: see tests/test_oracle_pins.py (P1-P11, P13-P15 of DESIGN.md).  Nothing is "parity unpinned".
+Pins: see tests/test_oracle_pins.py (P1-P11, P13-P16 of DESIGN.md).  Nothing is "parity unpinned".
 """
 from __future__ import annotations
 
@@ -498,3 +498,19 @@ def gaussian_beam_g(k, w, r_G, alpha, beta, alpha_G=0.0, E0=1.0) -> np.ndarray:
     amp = E0 * k * k * w * w / (4 * np.pi) * np.cos(beta) * np.exp(-w * w * k * k * np.sin(beta) ** 2 / 4.0)
     amp = np.where(beta <= np.pi / 2, amp, 0.0) * np.exp(-1j * (kvec @ np.asarray(r_G, dtype=np.float64)))
     return np.stack([amp * np.cos(alpha - alpha_G), amp * np.sin(alpha - alpha_G)], axis=1)
+
+
+# ----------------------------------------------------------------------------- near field (eq. 3)
+def scattered_field(pos, k, lmax, b, points) -> np.ndarray:
+    """E_scat(r) = sum_i sum_n b^i_n Psi^(3)_n(r - r_i), eq. (3), with svwf() ((A.2); pinned by P1, P2).
+    points [n_pts, 3] outside every sphere.  Returns [n_pts, 3] complex128 Cartesian components."""
+    pos = np.atleast_2d(np.asarray(pos, dtype=np.float64))
+    pts = np.atleast_2d(np.asarray(points, dtype=np.float64))
+    b = np.asarray(b, dtype=np.complex128).reshape(pos.shape[0], nmax_of(lmax))
+    E = np.zeros((pts.shape[0], 3), dtype=np.complex128)
+    idx = multi_indices(lmax)
+    for i in range(pos.shape[0]):
+        rel = pts - pos[i][None, :]
+        for n, (tau, l, m) in enumerate(idx):
+            E += b[i, n] * svwf(3, tau, l, m, k, rel)
+    return E

@@ -26,7 +26,8 @@ CELES_MAX_HISTORY = 4096
 EXPORTS = ["celes_setup", "celes_coupling_matvec", "celes_system_matvec", "celes_coupling_matvec_host",
            "celes_system_matvec_host", "celes_solve", "celes_destroy", "celes_strerror", "celes_nmax",
            "celes_launch_config", "celes_translation_table", "celes_fp32_peak_probe", "celes_precond_setup",
-           "celes_precond_apply", "celes_partition", "celes_far_field", "celes_gaussian_beam"]
+           "celes_precond_apply", "celes_partition", "celes_far_field", "celes_gaussian_beam",
+           "celes_scattered_field"]
 
 
 class CelesError(RuntimeError):
@@ -97,6 +98,8 @@ def lib() -> ctypes.CDLL:
         L.celes_precond_apply.argtypes = [p, p, p, p]
         L.celes_partition.restype = i
         L.celes_partition.argtypes = [i, p, p, p, ctypes.POINTER(i)]
+        L.celes_scattered_field.restype = i
+        L.celes_scattered_field.argtypes = [p, p, i, p, p, p]
         L.celes_gaussian_beam.restype = i
         L.celes_gaussian_beam.argtypes = [p, ctypes.POINTER(celes_beam), p, p]
         L.celes_far_field.restype = i
@@ -265,6 +268,21 @@ def celes_gaussian_beam(ctx: Context, waist: float, center, alpha_G: float = 0.0
     if rc != CELES_OK:
         raise CelesError(rc, "celes_gaussian_beam")
     return a_in
+
+
+def celes_scattered_field(ctx: Context, b, points, stream=None):
+    """E_scat [n_pts, 3] complex64 (device) at the host points [n_pts, 3]; celes_scattered_field of include/celes.h."""
+    import torch
+    _check_vec(b, ctx, "b")
+    pts = np.ascontiguousarray(points, dtype=np.float64)
+    if pts.ndim != 2 or pts.shape[1] != 3 or pts.shape[0] < 1:
+        raise ValueError("points: [n_pts, 3]")
+    E = torch.empty(pts.shape[0], 3, dtype=torch.complex64, device=b.device)
+    rc = lib().celes_scattered_field(ctx.handle, b.data_ptr(), int(pts.shape[0]), pts.ctypes.data, E.data_ptr(),
+                                     _stream(stream))
+    if rc != CELES_OK:
+        raise CelesError(rc, "celes_scattered_field")
+    return E
 
 
 def celes_far_field(ctx: Context, b, alpha, beta, g=None, stream=None):

@@ -21,6 +21,7 @@
 #include "far_field.cuh"
 #include "gaussian_beam.cuh"
 #include "krylov_kernels.cuh"
+#include "near_field.cuh"
 #include "partition.h"
 #include "precond_kernels.cuh"
 #include "translation_table.h"
@@ -991,6 +992,34 @@ int celes_gaussian_beam(celes_ctx* ctx, const celes_beam* beam, void* a_in_dev, 
     }
     if (cudaStreamSynchronize(s) != cudaSuccess && !rc) rc = CELES_ECUDA;
     cudaFree(d_sb); cudaFree(d_cb); cudaFree(d_cm); cudaFree(d_cp);
+    return rc;
+}
+
+int celes_scattered_field(celes_ctx* ctx, const void* b_dev, int n_pts, const double* pts_xyz, void* e_dev, void* cuda_stream) {
+    if (!ctx || !b_dev || !e_dev || !pts_xyz || n_pts < 1) return CELES_EINVAL;
+    for (long long t = 0; t < 3LL * n_pts; ++t) if (!std::isfinite(pts_xyz[t])) return CELES_EINVAL;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    std::vector<double> kp(3 * (size_t)n_pts);
+    for (size_t t = 0; t < kp.size(); ++t) kp[t] = ctx->k * pts_xyz[t];
+    double* d_pts = nullptr;
+    CU_TRY(cudaMalloc(&d_pts, sizeof(double) * kp.size()));
+    int rc = CELES_OK;
+    if (cudaMemcpyAsync(d_pts, kp.data(), sizeof(double) * kp.size(), cudaMemcpyHostToDevice, s) != cudaSuccess) rc = CELES_ECUDA;
+    if (!rc) {
+        const int grid = (n_pts + celes::kNearThreads - 1) / celes::kNearThreads;
+        const float2* b = (const float2*)b_dev;
+        float2* E = (float2*)e_dev;
+        switch (ctx->lmax) {
+            case 1: celes::near_field_kernel<1><<<grid, celes::kNearThreads, 0, s>>>(ctx->N, n_pts, ctx->kpos, b, d_pts, E); break;
+            case 2: celes::near_field_kernel<2><<<grid, celes::kNearThreads, 0, s>>>(ctx->N, n_pts, ctx->kpos, b, d_pts, E); break;
+            case 3: celes::near_field_kernel<3><<<grid, celes::kNearThreads, 0, s>>>(ctx->N, n_pts, ctx->kpos, b, d_pts, E); break;
+            case 4: celes::near_field_kernel<4><<<grid, celes::kNearThreads, 0, s>>>(ctx->N, n_pts, ctx->kpos, b, d_pts, E); break;
+            default: rc = CELES_EINVAL;
+        }
+        if (!rc && cudaGetLastError() != cudaSuccess) rc = CELES_ECUDA;
+    }
+    if (cudaStreamSynchronize(s) != cudaSuccess && !rc) rc = CELES_ECUDA;
+    cudaFree(d_pts);
     return rc;
 }
 

@@ -412,3 +412,26 @@ def test_solve_warm_start_from_x0():
     warm = celes.celes_solve(ctx, a_dev, rough, rtol=1e-5)
     assert warm["converged"] and warm["iterations"] < cold["iterations"]
     assert rel(rough.cpu().numpy(), x.cpu().numpy()) <= 1e-3
+
+
+@pytest.mark.parametrize("lmax", [1, 2, 3, 4])
+def test_scattered_field_matches_oracle(lmax):
+    """celes_scattered_field (eq. 3 with (A.2)) against the oracle at points outside every sphere: random points in
+    and around the slab (some 5 nm from a surface), points exactly above sphere centres (rho = 0), every lmax."""
+    import dataclasses
+    w = dataclasses.replace(workloads.scaled(workloads.C3, 150), lmax=lmax)
+    pos, rad, q, ctx, b = make(w)
+    rng = np.random.default_rng(407)
+    lo, hi = pos.min(axis=0) - 300.0, pos.max(axis=0) + 300.0
+    pts = []
+    while len(pts) < 120:
+        p = rng.uniform(lo, hi)
+        if np.all(np.linalg.norm(pos - p, axis=1) > rad + 5.0):
+            pts.append(p)
+    pts += [pos[3] + np.array([0.0, 0.0, rad[3] + 40.0]), pos[7] - np.array([0.0, 0.0, rad[7] + 25.0])]
+    pts = np.array(pts)
+    E = celes.celes_scattered_field(ctx, torch.from_numpy(b).cuda(), pts).cpu().numpy()
+    ref = orc.scattered_field(pos, w.k, w.lmax, b, pts)
+    assert E.shape == (122, 3)
+    assert rel(E, ref) <= MATVEC_TOL
+    assert np.max(np.abs(E - ref)) <= 1e-3 * np.max(np.abs(ref))

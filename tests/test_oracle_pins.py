@@ -439,3 +439,34 @@ def test_p15_gaussian_beam_coefficients():
     flux = np.sum(W.ravel()[:, None] * np.abs(g) ** 2)                      # int sum_j |g_j|^2 sin(beta) d(beta) d(alpha)
     d5 = K**4 * w**4 / (8 * np.pi) * np.sum(wbeta * np.sin(beta) * np.cos(beta) ** 2 * np.exp(-w * w * K * K * np.sin(beta) ** 2 / 2))
     assert flux == pytest.approx(d5, rel=1e-12)                             # (D.5) / (2 pi^2 / (omega k mu_0))
+
+
+# --------------------------------------------------------------------------- P16 near field (eq. 3)
+def test_p16_scattered_field_is_consistent_with_far_field_and_translation():
+    """scattered_field() sums svwf() (pinned by P1, P2) over spheres.  Independent checks of the sum: (a) far from the
+    cluster it tends to the spherical wave of the plane-wave amplitudes g_j of P14 (A.12 evaluated by stationary phase:
+    E -> -2 pi i e^{ikr}/(kr) sum_j g_j e_j), which ties eq. (3) to (A.12)/(A.14) including the per-sphere phase;
+    (b) one sphere's outgoing field re-expanded about a second origin with the oracle's W block (eq. 7) gives the
+    same field near that origin."""
+    rng = np.random.default_rng(5)
+    b = rng.normal(size=(3, 30)) + 1j * rng.normal(size=(3, 30))
+    al, be = np.array([0.3, 2.0, 4.4]), np.array([0.5, 1.7, 2.6])
+    rhat = np.stack([np.sin(be) * np.cos(al), np.sin(be) * np.sin(al), np.cos(be)], axis=1)
+    R = 5.0e7                                                    # k R ~ 5.7e5: far field
+    E = o.scattered_field(POS3, K, 3, b, R * rhat)
+    g = o.far_field_amplitude(POS3, K, 3, b, al, be)
+    e_al = np.stack([-np.sin(al), np.cos(al), np.zeros(3)], axis=1)
+    e_be = np.stack([np.cos(be) * np.cos(al), np.cos(be) * np.sin(al), -np.sin(be)], axis=1)
+    Eff = (-2j * np.pi * np.exp(1j * K * R) / (K * R))[..., None] * (g[:, 0:1] * e_al + g[:, 1:2] * e_be)
+    assert np.max(np.abs(E - Eff)) <= 1e-4 * np.max(np.abs(Eff))
+    # (b)
+    d = POS3[1] - POS3[0]
+    b0 = np.zeros((1, 30), dtype=np.complex128)
+    b0[0] = b[0]
+    pts = POS3[1][None, :] + np.array([[6.0, -3.5, 4.5], [-2.5, 7.0, 1.5]])
+    E_direct = o.scattered_field(POS3[0:1], K, 3, b0, pts)
+    a_loc = o.coupling_block(3, K, d) @ b[0]                      # regular coefficients about sphere 1, lmax = 3
+    E_loc = np.zeros((2, 3), dtype=np.complex128)
+    for n, (tau, l, m) in enumerate(o.multi_indices(3)):
+        E_loc += a_loc[n] * o.svwf(1, tau, l, m, K, pts - POS3[1][None, :])
+    assert np.max(np.abs(E_loc - E_direct)) <= 5e-4 * np.max(np.abs(E_direct))     # truncation of the regular series at l = 3

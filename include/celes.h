@@ -35,7 +35,7 @@ extern "C" {
 #define CELES_ENOCONV -4   /* celes_solve reached max_iters; x holds the last iterate and info is filled */
 
 #define CELES_LMAX_MIN 1
-#define CELES_LMAX_MAX 4
+#define CELES_LMAX_MAX 5   /* lmax = 5 (nmax = 70): CELES_TRANSLATION_ROTATED only */
 #define CELES_MAX_HISTORY 4096
 
 typedef struct celes_ctx celes_ctx;   /* opaque; owns every device table; freed by celes_destroy */

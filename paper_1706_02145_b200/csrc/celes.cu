@@ -113,6 +113,7 @@ int prepare_coupling_t(celes_ctx* c, int* ctas_per_sm) {
         case 6: return fn<2, 0>(__VA_ARGS__); case 7: return fn<2, 1>(__VA_ARGS__); case 8: return fn<2, 2>(__VA_ARGS__);    \
         case 9: return fn<3, 0>(__VA_ARGS__); case 10: return fn<3, 1>(__VA_ARGS__); case 11: return fn<3, 2>(__VA_ARGS__);  \
         case 12: return fn<4, 0>(__VA_ARGS__); case 13: return fn<4, 1>(__VA_ARGS__); case 14: return fn<4, 2>(__VA_ARGS__); \
+        case 15: return fn<5, 0>(__VA_ARGS__);   /* lmax = 5: packed rotated body only */                            \
     }                                                                                                        \
     return CELES_EINVAL
 
@@ -369,6 +370,7 @@ int celes_setup(celes_ctx** out, int N, int lmax, const double* pos_xyz, const d
     if (!skip && !spheres_disjoint(N, pos_xyz, radii)) return CELES_EINVAL;
     if (opt && (opt->emitter_tile < 0 || opt->emitter_splits < 0 || opt->emitter_tile > 128)) return CELES_EINVAL;
     if (opt && (opt->translation < 0 || opt->translation > CELES_TRANSLATION_ROTATED_SCALAR)) return CELES_EINVAL;
+    if (lmax > 4 && opt && opt->translation != CELES_TRANSLATION_ROTATED) return CELES_EINVAL;   // one body at lmax = 5
     const bool table = opt && opt->hankel == CELES_HANKEL_TABLE;
     if (opt && opt->hankel != CELES_HANKEL_REGISTERS && opt->hankel != CELES_HANKEL_TABLE) return CELES_EINVAL;
     if (table && (opt->translation != CELES_TRANSLATION_ROTATED || !(opt->hankel_dr >= 0.0) || !std::isfinite(opt->hankel_dr)))
@@ -852,6 +854,7 @@ int celes_precond_setup(celes_ctx* ctx, const double* edge_xyz, celes_precond_in
             case 2: PC_ASM(2); break;
             case 3: PC_ASM(3); break;
             case 4: PC_ASM(4); break;
+            case 5: PC_ASM(5); break;
             default: return cleanup(CELES_EINVAL);
         }
 #undef PC_ASM
@@ -953,6 +956,7 @@ int celes_far_field(celes_ctx* ctx, const void* b_dev, int n_dir, const double* 
             case 2: celes::far_field_kernel<16><<<grid, celes::kFarThreads, 0, s>>>(ctx->N, chunk, rows, ctx->kpos, b, d_coef, d_dir, d_part); break;
             case 3: celes::far_field_kernel<30><<<grid, celes::kFarThreads, 0, s>>>(ctx->N, chunk, rows, ctx->kpos, b, d_coef, d_dir, d_part); break;
             case 4: celes::far_field_kernel<48><<<grid, celes::kFarThreads, 0, s>>>(ctx->N, chunk, rows, ctx->kpos, b, d_coef, d_dir, d_part); break;
+            case 5: celes::far_field_kernel<70><<<grid, celes::kFarThreads, 0, s>>>(ctx->N, chunk, rows, ctx->kpos, b, d_coef, d_dir, d_part); break;
             default: rc = CELES_EINVAL;
         }
         if (!rc) celes::far_field_reduce_kernel<<<(rows + 255) / 256, 256, 0, s>>>(rows, splits, d_part, (float2*)g_dev);
@@ -1014,6 +1018,7 @@ int celes_scattered_field(celes_ctx* ctx, const void* b_dev, int n_pts, const do
             case 2: celes::near_field_kernel<2><<<grid, celes::kNearThreads, 0, s>>>(ctx->N, n_pts, ctx->kpos, b, d_pts, E); break;
             case 3: celes::near_field_kernel<3><<<grid, celes::kNearThreads, 0, s>>>(ctx->N, n_pts, ctx->kpos, b, d_pts, E); break;
             case 4: celes::near_field_kernel<4><<<grid, celes::kNearThreads, 0, s>>>(ctx->N, n_pts, ctx->kpos, b, d_pts, E); break;
+            case 5: celes::near_field_kernel<5><<<grid, celes::kNearThreads, 0, s>>>(ctx->N, n_pts, ctx->kpos, b, d_pts, E); break;
             default: rc = CELES_EINVAL;
         }
         if (!rc && cudaGetLastError() != cudaSuccess) rc = CELES_ECUDA;

@@ -113,6 +113,8 @@ template <int LMAX>
 struct YPolicy { using type = YRegs<nmax_of(LMAX)>; };
 template <>
 struct YPolicy<4> { using type = YSmem<nmax_of(4)>; };
+template <>
+struct YPolicy<5> { using type = YSmem<nmax_of(5)>; };
 
 template <int LMAX>
 constexpr size_t coupling_smem_bytes(int etile) {

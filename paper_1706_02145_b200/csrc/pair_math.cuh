@@ -43,6 +43,7 @@ struct PairBodyPk;    // packed (FFMA2) rotate / axial-translate / rotate varian
 #include "generated/coupling_pk_lmax2.inc"
 #include "generated/coupling_pk_lmax3.inc"
 #include "generated/coupling_pk_lmax4.inc"
+#include "generated/coupling_pk_lmax5.inc"
 
 // How W^{ii'} b^{i'} is evaluated per pair (celes.h: CELES_TRANSLATION_*)
 namespace celes {

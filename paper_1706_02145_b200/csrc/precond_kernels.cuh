@@ -12,7 +12,7 @@
 
 namespace celes {
 
-constexpr int kAsmThreads = 64;     // >= nmax of every supported lmax (48 at lmax = 4)
+constexpr int kAsmThreads = 96;     // >= nmax of every supported lmax (70 at lmax = 5)
 constexpr int kGemvRows = 128;      // rows of a block handled by one CTA of block_gemv_kernel
 
 // One CTA per ordered pair (a, b) of spheres of one subset; thread t < nmax fills column n' = t of the nmax x nmax

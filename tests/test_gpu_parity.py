@@ -435,3 +435,38 @@ def test_scattered_field_matches_oracle(lmax):
     assert E.shape == (122, 3)
     assert rel(E, ref) <= MATVEC_TOL
     assert np.max(np.abs(E - ref)) <= 1e-3 * np.max(np.abs(ref))
+
+
+def test_lmax5_every_entry_point():
+    """lmax = 5 (nmax = 70; SURVEY.md section 8(f) row 2 asks for lmax >= 5 instantiations): larger spheres (R = 250 nm,
+    kR = 2.9) in a cube; coupling / system matvec, solve, preconditioner, far field, near field and beam coefficients
+    against the oracle.  Only the default translation exists at lmax = 5."""
+    import dataclasses
+    w = dataclasses.replace(workloads.scaled(workloads.C2, 40), lmax=5, radius_lo=230.0, radius_hi=270.0)
+    pos, rad, q, ctx, b = make(w)
+    assert w.nmax == 70
+    qo = orc.mie_q(w.lmax, w.k, rad, workloads.N_SPHERE)
+    ref = orc.coupling_matvec(pos, w.k, w.lmax, b)
+    bd = torch.from_numpy(b).cuda()
+    assert rel(gpu_coupling(ctx, b), ref) <= MATVEC_TOL
+    out = celes.celes_system_matvec(ctx, bd).cpu().numpy()
+    assert rel(out, b.astype(np.complex128) - orc.t_diagonal(qo, w.lmax) * ref) <= MATVEC_TOL
+    with pytest.raises(celes.CelesError):
+        celes.celes_setup(pos, rad, q, w.k, w.lmax, translation="direct")
+    a_in = orc.plane_wave_a_in(pos, w.k, w.lmax)
+    x = torch.zeros(w.N, w.nmax, dtype=torch.complex64, device="cuda")
+    info = celes.celes_solve(ctx, torch.from_numpy(a_in.astype(np.complex64)).cuda(), x, rtol=1e-4, max_iters=2000)
+    assert info["converged"]
+    assert rel(x.cpu().numpy(), orc.solve_dense(pos, w.k, w.lmax, qo, a_in)) <= SOLVE_TOL
+    celes.celes_precond_setup(ctx, 1500.0)
+    z = celes.celes_precond_apply(ctx, bd).cpu().numpy()
+    assert rel(z, orc.precond_apply(pos, w.k, w.lmax, qo, 1500.0, b)) <= SOLVE_TOL
+    al, be = np.array([0.0, 1.0, 4.0, 2.2]), np.array([0.0, 0.7, 2.9, np.pi / 2])
+    g = celes.celes_far_field(ctx, bd, al, be).cpu().numpy()
+    assert rel(g, orc.far_field_amplitude(pos, w.k, w.lmax, b, al, be)) <= MATVEC_TOL
+    pts = pos[:6] + np.array([0.0, 0.0, 1.0])[None, :] * (rad[:6, None] + 60.0)
+    pts = pts[[np.all(np.linalg.norm(pos - p, axis=1) > rad + 5.0) for p in pts]]
+    E = celes.celes_scattered_field(ctx, bd, pts).cpu().numpy()
+    assert rel(E, orc.scattered_field(pos, w.k, w.lmax, b, pts)) <= MATVEC_TOL
+    a = celes.celes_gaussian_beam(ctx, 1500.0, [0.0, 0.0, 0.0], 0.2, 1.0, n_beta=200).cpu().numpy()
+    assert rel(a, orc.gaussian_beam_a_in(pos, w.k, w.lmax, 1500.0, [0.0, 0.0, 0.0], 0.2, 1.0, n_beta=200)) <= 1e-6

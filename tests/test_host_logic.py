@@ -32,11 +32,11 @@ def test_library_exports_every_declared_symbol():
 
 
 def test_nmax_and_strerror():
-    assert [celes.celes_nmax(l) for l in (1, 2, 3, 4)] == [6, 16, 30, 48]
+    assert [celes.celes_nmax(l) for l in (1, 2, 3, 4, 5)] == [6, 16, 30, 48, 70]
     with pytest.raises(celes.CelesError):
         celes.celes_nmax(0)
     with pytest.raises(celes.CelesError):
-        celes.celes_nmax(5)
+        celes.celes_nmax(6)
     for code in (0, -1, -2, -3, -4):
         assert binding.strerror(code) and "unknown" not in binding.strerror(code)
     assert "unknown" in binding.strerror(-99)
@@ -89,7 +89,7 @@ def test_compute_entry_points_reject_null():
     L.celes_destroy(None)
 
 
-@pytest.mark.parametrize("lmax", [1, 2, 3, 4])
+@pytest.mark.parametrize("lmax", [1, 2, 3, 4, 5])
 def test_translation_table_matches_oracle_a5_b5(lmax):
     """The library's run-time table (own 3j code) against the oracle's Racah-formula a5/b5, with the index swap
     of eq. (7): W_{(lm),(l'm')} uses a5(l',m'|l,m|p)."""

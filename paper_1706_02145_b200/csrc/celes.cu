@@ -42,6 +42,7 @@ struct celes_ctx {
     HankelTable htab_desc = {nullptr, 0.0f, 0.0f, 0};
     float2* bpm = nullptr;       // [N][nmax] work: [b_+ | b_-]
     float2* ypart = nullptr;     // [splits][N][nmax] work: partial sums of the emitter splits
+    float2 *host_in = nullptr, *host_out = nullptr;   // [N][nmax] staging of the *_host entry points (allocated on first use)
     // Krylov work space (allocated on the first celes_solve)
     int kry_restart = 0, dot_blocks = 0;
     float2* V = nullptr;         // [restart+1][n] basis
@@ -192,7 +193,7 @@ void free_precond(celes_ctx* c) {
 void free_ctx(celes_ctx* c) {
     if (!c) return;
     free_precond(c);
-    cudaFree(c->kpos); cudaFree(c->tdiag); cudaFree(c->bpm); cudaFree(c->ypart); cudaFree(c->htab);
+    cudaFree(c->kpos); cudaFree(c->tdiag); cudaFree(c->bpm); cudaFree(c->ypart); cudaFree(c->htab); cudaFree(c->host_in); cudaFree(c->host_out);
     cudaFree(c->V); cudaFree(c->rhs); cudaFree(c->tmp); cudaFree(c->partial); cudaFree(c->coef); cudaFree(c->hsum);
     if (c->hhost) cudaFreeHost(c->hhost);
     delete c;
@@ -498,15 +499,15 @@ static int matvec_host(celes_ctx* ctx, const void* b_host, void* y_host, bool sy
     if (!ctx || !b_host || !y_host) return CELES_EINVAL;
     cudaStream_t s = (cudaStream_t)cuda_stream;
     const size_t bytes = sizeof(float2) * (size_t)ctx->N * ctx->nmax;
-    float2 *bd = nullptr, *yd = nullptr;
-    CU_TRY(cudaMalloc(&bd, bytes));
-    if (cudaMalloc(&yd, bytes) != cudaSuccess) { cudaFree(bd); return CELES_ENOMEM; }
+    if (!ctx->host_in) {                       // device staging buffers of the host entry points, kept with the context
+        CU_TRY(cudaMalloc(&ctx->host_in, bytes));
+        if (cudaMalloc(&ctx->host_out, bytes) != cudaSuccess) { cudaFree(ctx->host_in); ctx->host_in = nullptr; return CELES_ENOMEM; }
+    }
     int rc = CELES_OK;
-    if (cudaMemcpyAsync(bd, b_host, bytes, cudaMemcpyHostToDevice, s) != cudaSuccess) rc = CELES_ECUDA;
-    if (!rc) rc = run_matvec(ctx, bd, yd, system, s);
-    if (!rc && cudaMemcpyAsync(y_host, yd, bytes, cudaMemcpyDeviceToHost, s) != cudaSuccess) rc = CELES_ECUDA;
+    if (cudaMemcpyAsync(ctx->host_in, b_host, bytes, cudaMemcpyHostToDevice, s) != cudaSuccess) rc = CELES_ECUDA;
+    if (!rc) rc = run_matvec(ctx, ctx->host_in, ctx->host_out, system, s);
+    if (!rc && cudaMemcpyAsync(y_host, ctx->host_out, bytes, cudaMemcpyDeviceToHost, s) != cudaSuccess) rc = CELES_ECUDA;
     if (cudaStreamSynchronize(s) != cudaSuccess && !rc) rc = CELES_ECUDA;
-    cudaFree(bd); cudaFree(yd);
     return rc;
 }
 

@@ -57,7 +57,7 @@ def test_setup_rejects_bad_arguments_before_touching_the_gpu():
     assert _setup_rc(2, 3, pos, rad, q, k, out=False)[0] == binding.CELES_EINVAL
     assert _setup_rc(0, 3, pos, rad, q, k) == (binding.CELES_EINVAL, None)
     assert _setup_rc(2, 0, pos, rad, q, k)[0] == binding.CELES_EINVAL
-    assert _setup_rc(2, 5, pos, rad, q, k)[0] == binding.CELES_EINVAL
+    assert _setup_rc(2, 6, pos, rad, q, k)[0] == binding.CELES_EINVAL
     assert _setup_rc(2, 3, None, rad, q, k)[0] == binding.CELES_EINVAL
     assert _setup_rc(2, 3, pos, None, q, k)[0] == binding.CELES_EINVAL
     assert _setup_rc(2, 3, pos, rad, None, k)[0] == binding.CELES_EINVAL

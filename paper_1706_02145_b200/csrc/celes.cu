@@ -50,8 +50,9 @@ struct celes_ctx {
     float2* tmp = nullptr;       // [n]
     double2* partial = nullptr;  // [dot_blocks][restart+1]
     double2* coef = nullptr;     // [restart+2]
-    double2* hsum = nullptr;     // [restart+2]
-    double2* hhost = nullptr;    // pinned [restart+2]
+    double2* hsum = nullptr;     // [2][restart+2]
+    double2* hhost = nullptr;    // pinned [3][restart+2]: two Hessenberg-column halves + coefficient upload
+    cudaEvent_t kry_ev[2] = {nullptr, nullptr};   // 'Hessenberg column copied' events of the look-ahead Arnoldi loop
     // block-diagonal preconditioner (celes_precond_setup)
     bool pc_ready = false;
     int pc_groups = 0, pc_max_n = 0, pc_ctas = 0;
@@ -196,6 +197,7 @@ void free_ctx(celes_ctx* c) {
     cudaFree(c->kpos); cudaFree(c->tdiag); cudaFree(c->bpm); cudaFree(c->ypart); cudaFree(c->htab); cudaFree(c->host_in); cudaFree(c->host_out);
     cudaFree(c->V); cudaFree(c->rhs); cudaFree(c->tmp); cudaFree(c->partial); cudaFree(c->coef); cudaFree(c->hsum);
     if (c->hhost) cudaFreeHost(c->hhost);
+    for (int q = 0; q < 2; ++q) if (c->kry_ev[q]) cudaEventDestroy(c->kry_ev[q]);
     delete c;
 }
 
@@ -218,8 +220,10 @@ int ensure_krylov(celes_ctx* c, int restart) {
     CU_TRY(cudaMalloc(&c->tmp, sizeof(float2) * n));
     CU_TRY(cudaMalloc(&c->partial, sizeof(double2) * c->dot_blocks * (restart + 1)));
     CU_TRY(cudaMalloc(&c->coef, sizeof(double2) * (restart + 2)));
-    CU_TRY(cudaMalloc(&c->hsum, sizeof(double2) * (restart + 2)));
-    CU_TRY(cudaMallocHost(&c->hhost, sizeof(double2) * (restart + 2)));
+    CU_TRY(cudaMalloc(&c->hsum, sizeof(double2) * 2 * (restart + 2)));
+    CU_TRY(cudaMallocHost(&c->hhost, sizeof(double2) * 3 * (restart + 2)));
+    for (int q = 0; q < 2; ++q)
+        if (!c->kry_ev[q]) CU_TRY(cudaEventCreateWithFlags(&c->kry_ev[q], cudaEventDisableTiming));
     c->kry_restart = restart;
     return CELES_OK;
 }
@@ -228,7 +232,7 @@ int ensure_krylov(celes_ctx* c, int restart) {
 int device_dots(celes_ctx* c, long long n, int k, const float2* V, const float2* w, double2* out, double2* accum,
                 cudaStream_t s) {
     celes::multi_dot_kernel<<<c->dot_blocks, celes::kDotBlock, 0, s>>>(n, k, V, w, c->partial);
-    celes::dots_reduce_kernel<<<(k + 63) / 64, 64, 0, s>>>(c->dot_blocks, k, c->partial, out, accum);
+    celes::dots_reduce_kernel<<<k, celes::kReduceThreads, 0, s>>>(c->dot_blocks, k, c->partial, out, accum);
     return cudaGetLastError() == cudaSuccess ? CELES_OK : CELES_ECUDA;
 }
 
@@ -625,7 +629,8 @@ extern "C" {
 // Restarted GMRES (Saad & Schultz, the paper's ref. [26]) on M x = T a_in, unpreconditioned,
 // classical Gram-Schmidt with one re-orthogonalisation pass (CGS2): the j+1 inner products of a pass are ONE
 // kernel, their coefficients stay on the device for the update, and one small device->host copy per inner
-// iteration brings the Hessenberg column to the host, where Givens rotations track the residual estimate.
+// iteration brings the Hessenberg column to the host, where Givens rotations track the residual estimate; the
+// device work of the next column is enqueued before the host waits for that copy (one column of look-ahead).
 // The TRUE residual is recomputed at every restart and decides convergence (reading R14).
 int celes_solve(celes_ctx* ctx, const void* a_in_dev, void* x_dev, const celes_solve_opts* o, celes_solve_info* info,
                 void* cuda_stream) {
@@ -695,34 +700,57 @@ int celes_solve(celes_ctx* ctx, const void* a_in_dev, void* x_dev, const celes_s
         celes::scale_by_inv_norm_kernel<<<eb, 256, 0, s>>>(n, ctx->coef, V, V);
         std::fill(g.begin(), g.end(), cd(0.0));
         g[0] = beta;
-        int j = 0;
-        for (; j < restart && iterations < max_iters; ++j) {
-            float2* w = V + (size_t)(j + 1) * n;
+        // Arnoldi with one column of look-ahead: the device work of column j+1 (it only needs v_{j+1}, which is
+        // normalised on the device) is enqueued BEFORE the host waits for the Hessenberg column j, so the Givens
+        // update and the copy latency overlap the next matvec.  Convergence is seen one column late at worst:
+        // the column already enqueued is then simply not used.
+        const int hs = ctx->kry_restart + 2;                   // stride of the two hsum / hhost halves (as allocated)
+        auto enqueue_column = [&](int jc) -> int {
+            float2* w = V + (size_t)(jc + 1) * n;
+            double2* hsum = ctx->hsum + (size_t)(jc & 1) * hs;
+            int r2;
             if (pc) {                                          // right preconditioning: w = M (P^{-1} v_j)
-                rc = precond_apply(ctx, V + (size_t)j * n, ctx->pc_tmp, s);
-                if (rc) return finish(rc);
-                rc = run_matvec(ctx, ctx->pc_tmp, w, true, s);
+                r2 = precond_apply(ctx, V + (size_t)jc * n, ctx->pc_tmp, s);
+                if (r2) return r2;
+                r2 = run_matvec(ctx, ctx->pc_tmp, w, true, s);
             } else {
-                rc = run_matvec(ctx, V + (size_t)j * n, w, true, s);
+                r2 = run_matvec(ctx, V + (size_t)jc * n, w, true, s);
             }
-            if (rc) return finish(rc);
-            ++matvecs; ++iterations;
-            CU_TRY(cudaMemsetAsync(ctx->hsum, 0, sizeof(double2) * (j + 2), s));
+            if (r2) return r2;
+            ++matvecs;
+            CU_TRY(cudaMemsetAsync(hsum, 0, sizeof(double2) * (jc + 2), s));
             for (int pass = 0; pass < 2; ++pass) {
-                rc = device_dots(ctx, n, j + 1, V, w, ctx->coef, ctx->hsum, s);
-                if (rc) return finish(rc);
-                rc = device_axpys(ctx, n, j + 1, -1.0, ctx->coef, V, w, s);
-                if (rc) return finish(rc);
+                r2 = device_dots(ctx, n, jc + 1, V, w, ctx->coef, hsum, s);
+                if (r2) return r2;
+                r2 = device_axpys(ctx, n, jc + 1, -1.0, ctx->coef, V, w, s);
+                if (r2) return r2;
             }
-            rc = device_dots(ctx, n, 1, w, w, ctx->hsum + (j + 1), nullptr, s);
+            r2 = device_dots(ctx, n, 1, w, w, hsum + (jc + 1), nullptr, s);
+            if (r2) return r2;
+            celes::scale_by_inv_norm_kernel<<<eb, 256, 0, s>>>(n, hsum + (jc + 1), w, w);
+            CU_TRY(cudaMemcpyAsync(ctx->hhost + (size_t)(jc & 1) * hs, hsum, sizeof(double2) * (jc + 2), cudaMemcpyDeviceToHost, s));
+            CU_TRY(cudaEventRecord(ctx->kry_ev[jc & 1], s));
+            return CELES_OK;
+        };
+        int j = 0, enq = 0;
+        if (iterations < max_iters) {
+            rc = enqueue_column(0);
             if (rc) return finish(rc);
-            celes::scale_by_inv_norm_kernel<<<eb, 256, 0, s>>>(n, ctx->hsum + (j + 1), w, w);
-            CU_TRY(cudaMemcpyAsync(ctx->hhost, ctx->hsum, sizeof(double2) * (j + 2), cudaMemcpyDeviceToHost, s));
-            CU_TRY(cudaStreamSynchronize(s));
+            enq = 1;
+        }
+        while (j < enq) {
+            if (enq < restart && iterations + (enq - j) < max_iters) {      // look-ahead
+                rc = enqueue_column(enq);
+                if (rc) return finish(rc);
+                ++enq;
+            }
+            CU_TRY(cudaEventSynchronize(ctx->kry_ev[j & 1]));
+            ++iterations;
+            const double2* hh = ctx->hhost + (size_t)(j & 1) * hs;
             // Hessenberg column j, Givens rotations
             cd* col = &Hm[(size_t)j * (restart + 1)];
-            for (int i = 0; i <= j; ++i) col[i] = cd(ctx->hhost[i].x, ctx->hhost[i].y);
-            const double hnext = std::sqrt(std::max(0.0, ctx->hhost[j + 1].x));
+            for (int i = 0; i <= j; ++i) col[i] = cd(hh[i].x, hh[i].y);
+            const double hnext = std::sqrt(std::max(0.0, hh[j + 1].x));
             for (int i = 0; i < j; ++i) {
                 const cd t = cs[i] * col[i] + sn[i] * col[i + 1];
                 col[i + 1] = -std::conj(sn[i]) * col[i] + cs[i] * col[i + 1];
@@ -738,16 +766,18 @@ int celes_solve(celes_ctx* ctx, const void* a_in_dev, void* x_dev, const celes_s
             g[j] = cs[j] * g[j];
             const double est = std::abs(g[j + 1]) / fnorm;
             push_hist(est);
-            if (est <= rtol || hnext == 0.0) { ++j; break; }
+            ++j;
+            if (est <= rtol || hnext == 0.0) break;
         }
+        double2* hup = ctx->hhost + 2 * (size_t)hs;            // third part of the pinned buffer: coefficient upload
         // back substitution R y = g, x += V y
         for (int i = j - 1; i >= 0; --i) {
             cd acc = g[i];
             for (int q = i + 1; q < j; ++q) acc -= Hm[(size_t)q * (restart + 1) + i] * yv[q];
             yv[i] = acc / Hm[(size_t)i * (restart + 1) + i];
         }
-        for (int i = 0; i < j; ++i) ctx->hhost[i] = make_double2(yv[i].real(), yv[i].imag());
-        CU_TRY(cudaMemcpyAsync(ctx->coef, ctx->hhost, sizeof(double2) * j, cudaMemcpyHostToDevice, s));
+        for (int i = 0; i < j; ++i) hup[i] = make_double2(yv[i].real(), yv[i].imag());
+        CU_TRY(cudaMemcpyAsync(ctx->coef, hup, sizeof(double2) * j, cudaMemcpyHostToDevice, s));
         if (j > 0 && pc) {                                     // x += P^{-1} (V y)
             CU_TRY(cudaMemsetAsync(ctx->tmp, 0, sizeof(float2) * n, s));
             rc = device_axpys(ctx, n, j, 1.0, ctx->coef, V, ctx->tmp, s);

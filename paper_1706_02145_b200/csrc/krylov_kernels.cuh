@@ -53,14 +53,26 @@ __global__ void __launch_bounds__(kDotBlock) multi_dot_kernel(long long n, int k
 }
 
 // out[j] = sum_b partial[b][j]; if accum != nullptr also accum[j] += out[j] (CGS2: h = h1 + h2).
-__global__ void dots_reduce_kernel(int nblocks, int k, const double2* __restrict__ partial, double2* __restrict__ out,
-                                   double2* __restrict__ accum) {
-    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+// One CTA of kReduceThreads per inner product j: the nblocks partial sums are read in parallel (a serial loop over
+// them in one thread costs nblocks dependent L2 latencies, which dominated the Krylov overhead), summed in a fixed
+// order per thread, then by warp shuffles and a shared-memory pass -- deterministic.
+constexpr int kReduceThreads = 128;
+__global__ void __launch_bounds__(kReduceThreads) dots_reduce_kernel(int nblocks, int k, const double2* __restrict__ partial,
+                                                                     double2* __restrict__ out, double2* __restrict__ accum) {
+    __shared__ double sr[kReduceThreads / 32], si[kReduceThreads / 32];
+    const int j = blockIdx.x;
     if (j >= k) return;
     double r = 0.0, i = 0.0;
-    for (int b = 0; b < nblocks; ++b) { const double2 p = partial[(size_t)b * k + j]; r += p.x; i += p.y; }
-    out[j] = make_double2(r, i);
-    if (accum != nullptr) { accum[j].x += r; accum[j].y += i; }
+    for (int b = threadIdx.x; b < nblocks; b += kReduceThreads) { const double2 p = partial[(size_t)b * k + j]; r += p.x; i += p.y; }
+    r = warp_sum(r); i = warp_sum(i);
+    if ((threadIdx.x & 31) == 0) { sr[threadIdx.x >> 5] = r; si[threadIdx.x >> 5] = i; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double tr = 0.0, ti = 0.0;
+        for (int q = 0; q < kReduceThreads / 32; ++q) { tr += sr[q]; ti += si[q]; }
+        out[j] = make_double2(tr, ti);
+        if (accum != nullptr) { accum[j].x += tr; accum[j].y += ti; }
+    }
 }
 
 // w[t] += alpha * sum_{j<k} coef[j] * V_j[t]       (alpha = -1: orthogonalisation, +1: solution update)

@@ -470,3 +470,33 @@ def test_lmax5_every_entry_point():
     assert rel(E, orc.scattered_field(pos, w.k, w.lmax, b, pts)) <= MATVEC_TOL
     a = celes.celes_gaussian_beam(ctx, 1500.0, [0.0, 0.0, 0.0], 0.2, 1.0, n_beta=200).cpu().numpy()
     assert rel(a, orc.gaussian_beam_a_in(pos, w.k, w.lmax, 1500.0, [0.0, 0.0, 0.0], 0.2, 1.0, n_beta=200)) <= 1e-6
+
+
+def test_absorbing_spheres_solve_and_cross_sections():
+    """Complex refractive index (reading R10: Im n > 0 absorbs): the T diagonal is complex without the lossless
+    relation Re Q = -|Q|^2; system matvec and solve against the oracle, and extinction > scattering on the GPU
+    solution (far-field flux of celes_far_field against the oracle's C_ext)."""
+    w = workloads.scaled(workloads.C2, 80)
+    pos, rad = workloads.positions(w)
+    n_abs = 1.52 + 0.1j
+    q = fields.mie_coefficients(w.lmax, w.k, rad, n_abs)
+    qo = orc.mie_q(w.lmax, w.k, rad, n_abs)
+    ctx = celes.celes_setup(pos, rad, q, w.k, w.lmax)
+    b = workloads.gaussian_coefficients(w.N, w.nmax, w.seed_b)
+    out = celes.celes_system_matvec(ctx, torch.from_numpy(b).cuda()).cpu().numpy()
+    assert rel(out, orc.system_matvec(pos, w.k, w.lmax, qo, b)) <= MATVEC_TOL
+    a_in = orc.plane_wave_a_in(pos, w.k, w.lmax)
+    x = torch.zeros(w.N, w.nmax, dtype=torch.complex64, device="cuda")
+    info = celes.celes_solve(ctx, torch.from_numpy(a_in.astype(np.complex64)).cuda(), x, rtol=1e-5)
+    assert info["converged"]
+    xg = x.cpu().numpy().astype(np.complex128)
+    assert rel(xg, orc.solve_dense(pos, w.k, w.lmax, qo, a_in)) <= SOLVE_TOL
+    xb, wb = np.polynomial.legendre.leggauss(48)
+    na = 96
+    A, B = np.meshgrid(2 * np.pi * np.arange(na) / na, np.arccos(xb), indexing="ij")
+    W = np.broadcast_to(wb[None, :] * 2 * np.pi / na, A.shape).ravel()
+    g = celes.celes_far_field(ctx, x, A.ravel(), B.ravel()).cpu().numpy().astype(np.complex128)
+    csca = orc.scattered_power_cross_section(w.k, g, W)
+    cext = orc.extinction_cross_section(w.k, a_in, xg)
+    assert csca == pytest.approx(orc.scattering_cross_section(pos, w.k, w.lmax, xg), rel=2e-3)
+    assert cext > 1.2 * csca                                   # absorption takes the difference

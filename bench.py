@@ -33,16 +33,16 @@ METRIC = "sphere_pair_translations_per_s"
 UNIT = "pairs/s"
 # FP32 flops per ordered pair of the two pair bodies, counted in the SASS of the coupling kernel's loop body
 # (2 FFMA + FMUL + FADD): geometry + radial functions + rotation/translation + accumulation.
-FLOPS_PER_PAIR = {"rotated": {3: 1893.0, 4: 3769.0}, "rotated_scalar": {3: 2324.0, 4: 4844.0},
-                  "direct": {3: 5412.0, 4: 14238.0}}
+FLOPS_PER_PAIR = {"rotated": {3: 1878.0, 4: 3753.0}, "rotated_scalar": {3: 2312.0, 4: 4830.0},
+                  "direct": {3: 5390.0, 4: 14197.0}}
 # FP32 lane operations per pair (an FFMA2 / FMUL2 / FADD2 is two, an FFMA / FMUL / FADD one): the FMA pipe retires 128 per
 # SM per clock whatever their kind, so lane_ops x pairs / (128 x SMs x clock x time) is the pipe utilisation
-LANE_OPS_PER_PAIR = {"rotated": {3: 1223.0, 4: 2350.0}, "rotated_scalar": {3: 1377.0, 4: 2781.0},
-                     "direct": {3: 3042.0, 4: 7983.0}}
+LANE_OPS_PER_PAIR = {"rotated": {3: 1216.0, 4: 2342.0}, "rotated_scalar": {3: 1369.0, 4: 2771.0},
+                     "direct": {3: 3026.0, 4: 7959.0}}
 FP32_LANES_PER_SM = 128
 # dram__bytes_read.sum + dram__bytes_write.sum of one coupling-kernel launch, from the ncu --set full captures
-# summarised under profiles/ (r01c_packed_kernel_c4.md, r01b_rotated_kernel_c4.md)
-NCU_DRAM_BYTES_PER_LAUNCH = {("C4", "rotated"): 132.8e6, ("C4", "rotated_scalar"): 132.0e6}
+# summarised under profiles/ (r01h_final_kernel_c4.md, r01b_rotated_kernel_c4.md)
+NCU_DRAM_BYTES_PER_LAUNCH = {("C4", "rotated"): 131.4e6, ("C4", "rotated_scalar"): 132.0e6}
 
 
 def parse():

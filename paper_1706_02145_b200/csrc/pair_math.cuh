@@ -60,6 +60,21 @@ struct HankelTable {
     int last;              // index of the last node
 };
 
+// sin, cos of kd.  kd reaches ~1e3 rad, where the hardware approximations (MUFU.SIN / MUFU.COS behind __sincosf) are
+// useless on their own; after a Cody-Waite reduction to [-pi, pi] (2 pi = 6.28125 + 1.9353072e-3: the first product
+// n * 6.28125 is exact for n < 2^15) their absolute error is ~4e-7, far inside the 1e-4 budget, and the pair saves the
+// ~25 instructions of sincosf's polynomial path.  Define CELES_ACCURATE_SINCOS to get sincosf back.
+CELES_DEVICE void sincos_kd(float x, float* s, float* c) {
+#ifdef CELES_ACCURATE_SINCOS
+    sincosf(x, s, c);
+#else
+    const float n = rintf(x * 0.15915494309189535f);
+    float r = fmaf(n, -6.28125f, x);
+    r = fmaf(n, -1.9353071795864769e-3f, r);
+    __sincosf(r, s, c);
+#endif
+}
+
 // dx, dy, dz: components of k (r_i - r_i') (dimensionless), already rounded to FP32 AFTER the subtraction
 // was done in FP64 (coordinate rounding is the dominant FP32 error otherwise).
 // bload(q): emitter coefficient q in the variant's work basis;  yacc: accumulator policy of the receiver.
@@ -96,7 +111,7 @@ CELES_DEVICE void pair_translate(float dx, float dy, float dz, const HankelTable
         return;
     }
     float sx, cx;
-    sincosf(x, &sx, &cx);                            // full-range accurate: kd reaches ~1000 rad
+    sincos_kd(x, &sx, &cx);                          // kd reaches ~1000 rad: reduced first
     if constexpr (VARIANT == celes::kRotated) {             // the same recurrence on packed (Re, Im)
         float2 h[P];
         h[0] = mul2(bc2(rinv), make_float2(sx, -cx));

@@ -131,7 +131,7 @@ __global__ void __launch_bounds__(kFarThreads) far_field_kernel(int N, int chunk
             double ph = -(nx * spos[3 * e] + ny * spos[3 * e + 1] + nz * spos[3 * e + 2]);
             ph -= 6.283185307179586476925 * rint(ph * 0.15915494309189533577);
             float sn, cs;
-            sincosf((float)ph, &sn, &cs);
+            __sincosf((float)ph, &sn, &cs);                         // |ph| <= pi after the FP64 reduction: hardware path
             const float4* be = reinterpret_cast<const float4*>(sb + e * NMAX);
             // sum_n c_n b_n = P + i Q, two independent chains each
             float2 P0 = make_float2(0.f, 0.f), Q0 = P0, P1 = P0, Q1 = P0;

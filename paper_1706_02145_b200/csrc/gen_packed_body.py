@@ -111,7 +111,7 @@ def bcast(sign, var):
     return f"bc2({'-' if sign < 0 else ''}{var})"
 
 
-def emit(lmax):
+def emit(lmax, outdir=None):
     H = lmax * (lmax + 2)
     P = 2 * lmax + 1
     out = []
@@ -275,8 +275,9 @@ def emit(lmax):
         w("    }")
     w("  }")
     w("};")
-    os.makedirs(os.path.join(HERE, "generated"), exist_ok=True)
-    path = os.path.join(HERE, "generated", f"coupling_pk_lmax{lmax}.inc")
+    outdir = outdir or os.path.join(HERE, "generated")
+    os.makedirs(outdir, exist_ok=True)
+    path = os.path.join(outdir, f"coupling_pk_lmax{lmax}.inc")
     with open(path, "w") as f:
         f.write("\n".join(out) + "\n")
     print(f"lmax={lmax}: {len(ent.defs)} unique rotation entries ({ent.n_ops} scalar ops), "

@@ -141,7 +141,7 @@ def axial_tables(lmax):
     return coef
 
 
-def emit(lmax):
+def emit(lmax, outdir=None):
     H = lmax * (lmax + 2)
     P = 2 * lmax + 1
     out = []
@@ -285,8 +285,9 @@ def emit(lmax):
         w("    }")
     w("  }")
     w("};")
-    os.makedirs(os.path.join(HERE, "generated"), exist_ok=True)
-    path = os.path.join(HERE, "generated", f"coupling_rot_lmax{lmax}.inc")
+    outdir = outdir or os.path.join(HERE, "generated")
+    os.makedirs(outdir, exist_ok=True)
+    path = os.path.join(outdir, f"coupling_rot_lmax{lmax}.inc")
     with open(path, "w") as f:
         f.write("\n".join(out) + "\n")
     print(f"lmax={lmax}: {nrot} rotation entries, {len(coef)} axial (l,l',m) entries -> {path}")

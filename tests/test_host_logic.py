@@ -4,6 +4,7 @@ the immediates baked into the generated kernel bodies, and the input-preparation
 import ctypes
 import os
 import re
+import sys
 
 import numpy as np
 import pytest
@@ -167,3 +168,21 @@ def test_partition_matches_oracle_cuboids():
             assert np.all(g[idx] == j)
     with pytest.raises(celes.CelesError):
         celes.celes_partition(np.array([[np.nan, 0.0, 0.0]]), 1.0)
+
+
+@pytest.mark.parametrize("gen,prefix", [("gen_coupling_body", "coupling_body"), ("gen_rotated_body", "coupling_rot"),
+                                        ("gen_packed_body", "coupling_pk")])
+def test_committed_generated_bodies_are_what_the_generators_write(gen, prefix, tmp_path):
+    """The straight-line pair bodies under csrc/generated/ are build inputs: regenerate lmax = 1, 2 (seconds, SymPy)
+    and compare byte for byte with the committed files."""
+    csrc = os.path.join(ROOT, "paper_1706_02145_b200", "csrc")
+    sys.path.insert(0, csrc)
+    try:
+        mod = __import__(gen)
+        for lmax in (1, 2):
+            mod.emit(lmax, outdir=str(tmp_path))
+            new = open(tmp_path / f"{prefix}_lmax{lmax}.inc").read()
+            old = open(os.path.join(csrc, "generated", f"{prefix}_lmax{lmax}.inc")).read()
+            assert new == old
+    finally:
+        sys.path.remove(csrc)

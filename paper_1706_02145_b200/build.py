@@ -3,7 +3,7 @@
     python -m paper_1706_02145_b200.build [--force] [--regen]
 
 ``--regen`` re-runs csrc/gen_coupling_body.py first (needs SymPy; the generated files are committed).
-nvcc cross-compiles without a GPU.  The library is loaded by ``paper_1706_02145_b200.binding`` via ctypes.
+nvcc cross-compiles without a GPU.  Four translation units (csrc/celes.cu, solve.cu, precond.cu, fields.cu).  The library is loaded by ``paper_1706_02145_b200.binding`` via ctypes.
 """
 from __future__ import annotations
 
@@ -39,7 +39,8 @@ def build(force: bool = False, regen: bool = False, verbose: bool = False) -> st
         subprocess.run([sys.executable, os.path.join(CSRC, "gen_coupling_body.py")], check=True)
     if force or stale():
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-        cmd = [nvcc, *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []), "-o", LIB, os.path.join(CSRC, "celes.cu"), *NVCC_LIBS]
+        units = [os.path.join(CSRC, f) for f in ("celes.cu", "solve.cu", "precond.cu", "fields.cu")]
+        cmd = [nvcc, *NVCC_FLAGS, "--threads", "4", *(["-Xptxas", "-v"] if verbose else []), "-o", LIB, *units, *NVCC_LIBS]
         subprocess.run(cmd, check=True)
     return LIB
 

@@ -244,13 +244,4 @@ __global__ void finalize_kernel(int N, int H, int splits, const float2* __restri
     out[o2] = y2;
 }
 
-// out = T a (diagonal), used for the right-hand side of eq. (8)
-__global__ void tapply_kernel(long long n, const float2* __restrict__ tdiag, const float2* __restrict__ a,
-                              float2* __restrict__ out) {
-    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (t >= n) return;
-    const float2 q = tdiag[t], v = a[t];
-    out[t] = make_float2(q.x * v.x - q.y * v.y, q.x * v.y + q.y * v.x);
-}
-
 }  // namespace celes

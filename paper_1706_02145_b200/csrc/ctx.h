@@ -1,0 +1,69 @@
+// ctx.h -- the context behind the opaque celes_ctx* of include/celes.h, and the few internal host functions that
+// the translation units of the library share (celes.cu: set-up and matvec; solve.cu: GMRES / BiCGSTAB; precond.cu:
+// block-diagonal preconditioner; fields.cu: Gaussian beam, far field, near field).
+#pragma once
+#include <cuda_runtime.h>
+
+#include <vector>
+
+#include "../../include/celes.h"
+#include "hankel_table.h"
+#include "variants.h"
+
+struct celes_ctx {
+    int N = 0, lmax = 0, nmax = 0;
+    double k = 0.0;
+    int device = 0, sm_count = 0;
+    int rblocks = 0, splits = 1, chunk = 0, etile = 32;
+    int variant = celes::kRotated;   // CELES_TRANSLATION_*: packed rotated (default), direct sum, scalar rotated
+    size_t coupling_smem = 0;
+    std::vector<double> pos;     // host copy of the centres [N][3] (partition of the preconditioner)
+    double* kpos = nullptr;      // [N][3] FP64, k * r_i
+    float2* tdiag = nullptr;     // [N][nmax] T diagonal Q^i_{tau,l} expanded over m (B.1)
+    float4* htab = nullptr;      // Hankel lookup table [nodes][2 lmax + 1] (CELES_HANKEL_TABLE), else null
+    HankelTable htab_desc = {nullptr, 0.0f, 0.0f, 0};
+    float2* bpm = nullptr;       // [N][nmax] work: [b_+ | b_-]
+    float2* ypart = nullptr;     // [splits][N][nmax] work: partial sums of the emitter splits
+    float2 *host_in = nullptr, *host_out = nullptr;   // [N][nmax] staging of the *_host entry points (allocated on first use)
+    // Krylov work space (allocated on the first celes_solve)
+    int kry_restart = 0, dot_blocks = 0;
+    float2* V = nullptr;         // [restart+1][n] basis
+    float2* rhs = nullptr;       // [n] T a_in
+    float2* tmp = nullptr;       // [n]
+    double2* partial = nullptr;  // [dot_blocks][restart+1]
+    double2* coef = nullptr;     // [restart+2]
+    double2* hsum = nullptr;     // [2][restart+2]
+    double2* hhost = nullptr;    // pinned [3][restart+2]: two Hessenberg-column halves + coefficient upload
+    cudaEvent_t kry_ev[2] = {nullptr, nullptr};   // 'Hessenberg column copied' events of the look-ahead Arnoldi loop
+    // block-diagonal preconditioner (celes_precond_setup)
+    bool pc_ready = false;
+    int pc_groups = 0, pc_max_n = 0, pc_ctas = 0;
+    long long pc_elems = 0;      // sum_j n_j^2
+    int* pc_order = nullptr;     // [N]
+    int* pc_grp_offset = nullptr;        // [groups+1]
+    long long* pc_blk_offset = nullptr;  // [groups]
+    int* pc_cta_group = nullptr;         // [pc_ctas]
+    int* pc_cta_row0 = nullptr;          // [pc_ctas]
+    float2* pc_blocks = nullptr;         // explicit inverses M_j^{-1}, column-major, back to back
+    float2* pc_tmp = nullptr;            // [n] work vector of the preconditioned solve
+};
+
+#define CU_TRY(expr)                                  \
+    do {                                              \
+        cudaError_t e_ = (expr);                      \
+        if (e_ != cudaSuccess) {                      \
+            return e_ == cudaErrorMemoryAllocation ? CELES_ENOMEM : CELES_ECUDA; \
+        }                                             \
+    } while (0)
+
+namespace celes {
+namespace host {
+// y = W b (system == false) or out = b - T (W b): pack -> coupling -> finalize, all on stream s (celes.cu)
+int run_matvec(celes_ctx* c, const float2* b, float2* out, bool system, cudaStream_t s);
+// z = blockdiag(M_j^{-1}) v, and release of the preconditioner (precond.cu)
+int precond_apply(celes_ctx* c, const float2* v, float2* z, cudaStream_t s);
+void free_precond(celes_ctx* c);
+// release of the Krylov work space (solve.cu)
+void free_krylov(celes_ctx* c);
+}  // namespace host
+}  // namespace celes

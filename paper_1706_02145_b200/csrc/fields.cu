@@ -1,0 +1,118 @@
+// fields.cu -- the steps either side of the solve: celes_gaussian_beam (Appendix C), celes_far_field (A.12, D.1-D.3)
+// and celes_scattered_field (eq. 3 with (A.2)).  Kernels in gaussian_beam.cuh, far_field.cuh, near_field.cuh.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <vector>
+
+#include "ctx.h"
+#include "packed_math.cuh"
+#include "far_field.cuh"
+#include "gaussian_beam.cuh"
+#include "near_field.cuh"
+
+extern "C" {
+
+int celes_far_field(celes_ctx* ctx, const void* b_dev, int n_dir, const double* alpha, const double* beta, void* g_dev,
+                    void* cuda_stream) {
+    if (!ctx || !b_dev || !g_dev || n_dir < 1 || !alpha || !beta || n_dir > (1 << 29)) return CELES_EINVAL;
+    for (int d = 0; d < n_dir; ++d)
+        if (!std::isfinite(alpha[d]) || !std::isfinite(beta[d])) return CELES_EINVAL;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const int nmax = ctx->nmax, rows = 2 * n_dir, gx = (rows + celes::kFarThreads - 1) / celes::kFarThreads;
+    // split the sphere sum so that the grid has about four CTAs per SM-slot pair, at least 4 tiles per CTA
+    int splits = std::max(1, std::min((8 * ctx->sm_count + gx - 1) / gx, std::max(1, ctx->N / (4 * celes::kFarTile))));
+    const int chunk = ((ctx->N + splits - 1) / splits + celes::kFarTile - 1) / celes::kFarTile * celes::kFarTile;
+    splits = (ctx->N + chunk - 1) / chunk;
+    double *d_ang = nullptr, *d_dir = nullptr;
+    float2 *d_coef = nullptr, *d_part = nullptr;
+    int rc = CELES_OK;
+    if (cudaMalloc(&d_ang, sizeof(double) * 2 * (size_t)n_dir) != cudaSuccess ||
+        cudaMalloc(&d_dir, sizeof(double) * 3 * (size_t)n_dir) != cudaSuccess ||
+        cudaMalloc(&d_coef, sizeof(float2) * (size_t)rows * nmax) != cudaSuccess ||
+        cudaMalloc(&d_part, sizeof(float2) * (size_t)rows * splits) != cudaSuccess) rc = CELES_ENOMEM;
+    if (!rc && (cudaMemcpyAsync(d_ang, alpha, sizeof(double) * n_dir, cudaMemcpyHostToDevice, s) != cudaSuccess ||
+                cudaMemcpyAsync(d_ang + n_dir, beta, sizeof(double) * n_dir, cudaMemcpyHostToDevice, s) != cudaSuccess)) rc = CELES_ECUDA;
+    if (!rc) {
+        celes::far_field_coefficients_kernel<<<(n_dir + 127) / 128, 128, 0, s>>>(ctx->lmax, n_dir, d_ang, d_ang + n_dir, d_coef, d_dir);
+        const float2* b = (const float2*)b_dev;
+        dim3 grid(gx, splits);
+        switch (ctx->lmax) {
+            case 1: celes::far_field_kernel<6><<<grid, celes::kFarThreads, 0, s>>>(ctx->N, chunk, rows, ctx->kpos, b, d_coef, d_dir, d_part); break;
+            case 2: celes::far_field_kernel<16><<<grid, celes::kFarThreads, 0, s>>>(ctx->N, chunk, rows, ctx->kpos, b, d_coef, d_dir, d_part); break;
+            case 3: celes::far_field_kernel<30><<<grid, celes::kFarThreads, 0, s>>>(ctx->N, chunk, rows, ctx->kpos, b, d_coef, d_dir, d_part); break;
+            case 4: celes::far_field_kernel<48><<<grid, celes::kFarThreads, 0, s>>>(ctx->N, chunk, rows, ctx->kpos, b, d_coef, d_dir, d_part); break;
+            case 5: celes::far_field_kernel<70><<<grid, celes::kFarThreads, 0, s>>>(ctx->N, chunk, rows, ctx->kpos, b, d_coef, d_dir, d_part); break;
+            default: rc = CELES_EINVAL;
+        }
+        if (!rc) celes::far_field_reduce_kernel<<<(rows + 255) / 256, 256, 0, s>>>(rows, splits, d_part, (float2*)g_dev);
+        if (!rc && cudaGetLastError() != cudaSuccess) rc = CELES_ECUDA;
+    }
+    if (cudaStreamSynchronize(s) != cudaSuccess && !rc) rc = CELES_ECUDA;
+    cudaFree(d_ang); cudaFree(d_dir); cudaFree(d_coef); cudaFree(d_part);
+    return rc;
+}
+
+int celes_gaussian_beam(celes_ctx* ctx, const celes_beam* beam, void* a_in_dev, void* cuda_stream) {
+    if (!ctx || !beam || !a_in_dev) return CELES_EINVAL;
+    const int n_beta = beam->n_beta > 0 ? beam->n_beta : 400;
+    if (!(beam->waist > 0.0) || !std::isfinite(beam->waist) || n_beta > 100000) return CELES_EINVAL;
+    for (int a = 0; a < 3; ++a) if (!std::isfinite(beam->center[a])) return CELES_EINVAL;
+    if (!std::isfinite(beam->alpha_G) || !std::isfinite(beam->E0_re) || !std::isfinite(beam->E0_im)) return CELES_EINVAL;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    std::vector<double> sb, cb;
+    std::vector<double2> cminus, cplus;
+    celes::gaussian_beam_tables(ctx->lmax, n_beta, ctx->k, beam->waist, sb, cb, cminus, cplus);
+    double *d_sb = nullptr, *d_cb = nullptr;
+    double2 *d_cm = nullptr, *d_cp = nullptr;
+    int rc = CELES_OK;
+    if (cudaMalloc(&d_sb, sizeof(double) * n_beta) != cudaSuccess || cudaMalloc(&d_cb, sizeof(double) * n_beta) != cudaSuccess ||
+        cudaMalloc(&d_cm, sizeof(double2) * cminus.size()) != cudaSuccess ||
+        cudaMalloc(&d_cp, sizeof(double2) * cplus.size()) != cudaSuccess) rc = CELES_ENOMEM;
+    if (!rc && (cudaMemcpyAsync(d_sb, sb.data(), sizeof(double) * n_beta, cudaMemcpyHostToDevice, s) != cudaSuccess ||
+                cudaMemcpyAsync(d_cb, cb.data(), sizeof(double) * n_beta, cudaMemcpyHostToDevice, s) != cudaSuccess ||
+                cudaMemcpyAsync(d_cm, cminus.data(), sizeof(double2) * cminus.size(), cudaMemcpyHostToDevice, s) != cudaSuccess ||
+                cudaMemcpyAsync(d_cp, cplus.data(), sizeof(double2) * cplus.size(), cudaMemcpyHostToDevice, s) != cudaSuccess)) rc = CELES_ECUDA;
+    if (!rc) {
+        const long long total = (long long)ctx->N * ctx->nmax;
+        celes::gaussian_beam_kernel<<<(unsigned)((total + 127) / 128), 128, 0, s>>>(
+            ctx->N, ctx->lmax, n_beta, ctx->kpos, ctx->k * beam->center[0], ctx->k * beam->center[1], ctx->k * beam->center[2],
+            beam->alpha_G, make_double2(beam->E0_re, beam->E0_im), d_sb, d_cb, d_cm, d_cp, (float2*)a_in_dev);
+        if (cudaGetLastError() != cudaSuccess) rc = CELES_ECUDA;
+    }
+    if (cudaStreamSynchronize(s) != cudaSuccess && !rc) rc = CELES_ECUDA;
+    cudaFree(d_sb); cudaFree(d_cb); cudaFree(d_cm); cudaFree(d_cp);
+    return rc;
+}
+
+int celes_scattered_field(celes_ctx* ctx, const void* b_dev, int n_pts, const double* pts_xyz, void* e_dev, void* cuda_stream) {
+    if (!ctx || !b_dev || !e_dev || !pts_xyz || n_pts < 1) return CELES_EINVAL;
+    for (long long t = 0; t < 3LL * n_pts; ++t) if (!std::isfinite(pts_xyz[t])) return CELES_EINVAL;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    std::vector<double> kp(3 * (size_t)n_pts);
+    for (size_t t = 0; t < kp.size(); ++t) kp[t] = ctx->k * pts_xyz[t];
+    double* d_pts = nullptr;
+    CU_TRY(cudaMalloc(&d_pts, sizeof(double) * kp.size()));
+    int rc = CELES_OK;
+    if (cudaMemcpyAsync(d_pts, kp.data(), sizeof(double) * kp.size(), cudaMemcpyHostToDevice, s) != cudaSuccess) rc = CELES_ECUDA;
+    if (!rc) {
+        const int grid = (n_pts + celes::kNearThreads - 1) / celes::kNearThreads;
+        const float2* b = (const float2*)b_dev;
+        float2* E = (float2*)e_dev;
+        switch (ctx->lmax) {
+            case 1: celes::near_field_kernel<1><<<grid, celes::kNearThreads, 0, s>>>(ctx->N, n_pts, ctx->kpos, b, d_pts, E); break;
+            case 2: celes::near_field_kernel<2><<<grid, celes::kNearThreads, 0, s>>>(ctx->N, n_pts, ctx->kpos, b, d_pts, E); break;
+            case 3: celes::near_field_kernel<3><<<grid, celes::kNearThreads, 0, s>>>(ctx->N, n_pts, ctx->kpos, b, d_pts, E); break;
+            case 4: celes::near_field_kernel<4><<<grid, celes::kNearThreads, 0, s>>>(ctx->N, n_pts, ctx->kpos, b, d_pts, E); break;
+            case 5: celes::near_field_kernel<5><<<grid, celes::kNearThreads, 0, s>>>(ctx->N, n_pts, ctx->kpos, b, d_pts, E); break;
+            default: rc = CELES_EINVAL;
+        }
+        if (!rc && cudaGetLastError() != cudaSuccess) rc = CELES_ECUDA;
+    }
+    if (cudaStreamSynchronize(s) != cudaSuccess && !rc) rc = CELES_ECUDA;
+    cudaFree(d_pts);
+    return rc;
+}
+
+}  // extern "C"

@@ -122,4 +122,19 @@ __global__ void lincomb_kernel(long long n, double2 a, const float2* __restrict_
     }
 }
 
+// out = T a (diagonal), used for the right-hand side of eq. (8)
+__global__ void tapply_kernel(long long n, const float2* __restrict__ tdiag, const float2* __restrict__ a,
+                              float2* __restrict__ out) {
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= n) return;
+    const float2 q = tdiag[t], v = a[t];
+    out[t] = make_float2(q.x * v.x - q.y * v.y, q.x * v.y + q.y * v.x);
+}
+
+// x += y
+__global__ void add_kernel(long long n, const float2* __restrict__ y, float2* __restrict__ x) {
+    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += (long long)gridDim.x * blockDim.x)
+        x[t] = make_float2(x[t].x + y[t].x, x[t].y + y[t].y);
+}
+
 }  // namespace celes

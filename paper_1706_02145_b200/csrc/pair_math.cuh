@@ -6,9 +6,9 @@
 // (generated/coupling_body_lmax*.inc, written by gen_coupling_body.py).
 #pragma once
 
-#ifndef CELES_DEVICE
-#define CELES_DEVICE __device__ __forceinline__
-#endif
+#include "hankel_table.h"
+#include "variants.h"
+#include "packed_math.cuh"
 
 template <int LMAX>
 struct PairBody;   // specialised by the generated files
@@ -26,16 +26,6 @@ struct PairBodyRot;   // rotate / axial-translate / rotate variant (gen_rotated_
 #include "generated/coupling_rot_lmax3.inc"
 #include "generated/coupling_rot_lmax4.inc"
 
-// Packed FP32 pairs (sm_100a: fma.rn.f32x2 / mul.rn.f32x2 / add.rn.f32x2 -> SASS FFMA2 / FMUL2 / FADD2).  A float2
-// holds one complex number (re, im); bc2(a) is the broadcast operand (a, a), which ptxas encodes as a scalar
-// register operand of FFMA2, and negations / swapped halves fold into operand modifiers.
-CELES_DEVICE float2 bc2(float a) { return make_float2(a, a); }
-CELES_DEVICE float2 neg2(float2 a) { return make_float2(-a.x, -a.y); }
-CELES_DEVICE float2 fma2(float2 a, float2 b, float2 c) { return __ffma2_rn(a, b, c); }
-CELES_DEVICE float2 mul2(float2 a, float2 b) { return __fmul2_rn(a, b); }
-CELES_DEVICE float2 add2(float2 a, float2 b) { return __fadd2_rn(a, b); }
-CELES_DEVICE float2 sub2(float2 a, float2 b) { return __fadd2_rn(a, neg2(b)); }
-
 template <int LMAX>
 struct PairBodyPk;    // packed (FFMA2) rotate / axial-translate / rotate variant (gen_packed_body.py)
 
@@ -45,35 +35,6 @@ struct PairBodyPk;    // packed (FFMA2) rotate / axial-translate / rotate varian
 #include "generated/coupling_pk_lmax4.inc"
 #include "generated/coupling_pk_lmax5.inc"
 
-// How W^{ii'} b^{i'} is evaluated per pair (celes.h: CELES_TRANSLATION_*)
-namespace celes {
-constexpr int kRotated = 0;         // packed FFMA2 rotate / axial-translate / rotate (default)
-constexpr int kDirect = 1;          // term-by-term sum of (A.6)-(A.8)
-constexpr int kRotatedScalar = 2;   // scalar-FFMA rotate / axial-translate / rotate
-}  // namespace celes
-
-// Spherical-Hankel lookup table of the paper's scheme: node j holds, for p = 0..2 lmax,
-// (Re h_p, Im h_p, dx Re h_p', dx Im h_p') at x_j = x0 + j dx; cubic Hermite interpolation between two nodes.
-struct HankelTable {
-    const float4* nodes;   // [n_nodes][P]
-    float x0, inv_dx;
-    int last;              // index of the last node
-};
-
-// sin, cos of kd.  kd reaches ~1e3 rad, where the hardware approximations (MUFU.SIN / MUFU.COS behind __sincosf) are
-// useless on their own; after a Cody-Waite reduction to [-pi, pi] (2 pi = 6.28125 + 1.9353072e-3: the first product
-// n * 6.28125 is exact for n < 2^15) their absolute error is ~4e-7, far inside the 1e-4 budget, and the pair saves the
-// ~25 instructions of sincosf's polynomial path.  Define CELES_ACCURATE_SINCOS to get sincosf back.
-CELES_DEVICE void sincos_kd(float x, float* s, float* c) {
-#ifdef CELES_ACCURATE_SINCOS
-    sincosf(x, s, c);
-#else
-    const float n = rintf(x * 0.15915494309189535f);
-    float r = fmaf(n, -6.28125f, x);
-    r = fmaf(n, -1.9353071795864769e-3f, r);
-    __sincosf(r, s, c);
-#endif
-}
 
 // dx, dy, dz: components of k (r_i - r_i') (dimensionless), already rounded to FP32 AFTER the subtraction
 // was done in FP64 (coordinate rounding is the dominant FP32 error otherwise).

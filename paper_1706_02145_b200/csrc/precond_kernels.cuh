@@ -164,10 +164,4 @@ __global__ void __launch_bounds__(kGemvRows) block_gemv_kernel(
     z[(size_t)order[g0 + s] * nmax + (r - s * nmax)] = make_float2(ar0 + ar1, ai0 + ai1);
 }
 
-// x += y
-__global__ void add_kernel(long long n, const float2* __restrict__ y, float2* __restrict__ x) {
-    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += (long long)gridDim.x * blockDim.x)
-        x[t] = make_float2(x[t].x + y[t].x, x[t].y + y[t].y);
-}
-
 }  // namespace celes

@@ -161,6 +161,14 @@ int celes_partition(int N, const double* pos_xyz, const double* edge_xyz, int* g
 int celes_far_field(celes_ctx* ctx, const void* b_dev, int n_dir, const double* alpha, const double* beta,
                     void* g_dev, void* cuda_stream);
 
+/* Initial-field coefficients of the plane wave E_0 Phi_j(alpha, beta; r) = E_0 exp(i k.r) e_j about every sphere centre,
+ * from (A.13)-(A.14): a^i_n = E_0 exp(i k.r_i) 4 exp(-i m alpha) B^dagger_nj(beta).
+ *   alpha, beta   azimuthal and polar angle of the wave vector, radians (beta = 0: propagation along +z).
+ *   polarisation  j = 1: along e_alpha (TE), j = 2: along e_beta (TM; x-polarised for alpha = beta = 0).
+ *   a_in_dev      device, N*nmax complex64.  Asynchronous on cuda_stream. */
+int celes_plane_wave(celes_ctx* ctx, double alpha, double beta, int polarisation, double E0_re, double E0_im,
+                     void* a_in_dev, void* cuda_stream);
+
 /* Gaussian beam of Appendix C: waist w centred at r_G, propagating along +z, field at the waist
  * E_0 (-sin alpha_G e_x + cos alpha_G e_y) exp(-((x-x_G)^2 + (y-y_G)^2)/w^2) (C.1). */
 typedef struct celes_beam {

@@ -26,7 +26,7 @@ CELES_MAX_HISTORY = 4096
 EXPORTS = ["celes_setup", "celes_coupling_matvec", "celes_system_matvec", "celes_coupling_matvec_host",
            "celes_system_matvec_host", "celes_solve", "celes_destroy", "celes_strerror", "celes_nmax",
            "celes_launch_config", "celes_translation_table", "celes_fp32_peak_probe", "celes_precond_setup",
-           "celes_precond_apply", "celes_partition", "celes_far_field", "celes_gaussian_beam",
+           "celes_precond_apply", "celes_partition", "celes_far_field", "celes_gaussian_beam", "celes_plane_wave",
            "celes_scattered_field"]
 
 
@@ -100,6 +100,8 @@ def lib() -> ctypes.CDLL:
         L.celes_partition.argtypes = [i, p, p, p, ctypes.POINTER(i)]
         L.celes_scattered_field.restype = i
         L.celes_scattered_field.argtypes = [p, p, i, p, p, p]
+        L.celes_plane_wave.restype = i
+        L.celes_plane_wave.argtypes = [p, d, d, i, d, d, p, p]
         L.celes_gaussian_beam.restype = i
         L.celes_gaussian_beam.argtypes = [p, ctypes.POINTER(celes_beam), p, p]
         L.celes_far_field.restype = i
@@ -252,6 +254,20 @@ def celes_precond_apply(ctx: Context, v, z=None, stream=None):
     if rc != CELES_OK:
         raise CelesError(rc, "celes_precond_apply")
     return z
+
+
+def celes_plane_wave(ctx: Context, alpha: float = 0.0, beta: float = 0.0, polarisation: int = 2, E0: complex = 1.0,
+                     a_in=None, stream=None):
+    """a_in [N, nmax] complex64 (device) of the plane wave E0 Phi_j(alpha, beta); celes_plane_wave of include/celes.h."""
+    import torch
+    if a_in is None:
+        a_in = torch.empty(ctx.N, ctx.nmax, dtype=torch.complex64, device="cuda")
+    _check_vec(a_in, ctx, "a_in")
+    rc = lib().celes_plane_wave(ctx.handle, float(alpha), float(beta), int(polarisation), float(complex(E0).real),
+                                float(complex(E0).imag), a_in.data_ptr(), _stream(stream))
+    if rc != CELES_OK:
+        raise CelesError(rc, "celes_plane_wave")
+    return a_in
 
 
 def celes_gaussian_beam(ctx: Context, waist: float, center, alpha_G: float = 0.0, E0: complex = 1.0, n_beta: int = 0,

@@ -54,6 +54,16 @@ int celes_far_field(celes_ctx* ctx, const void* b_dev, int n_dir, const double* 
     return rc;
 }
 
+int celes_plane_wave(celes_ctx* ctx, double alpha, double beta, int polarisation, double E0_re, double E0_im, void* a_in_dev,
+                     void* cuda_stream) {
+    if (!ctx || !a_in_dev || (polarisation != 1 && polarisation != 2)) return CELES_EINVAL;
+    if (!std::isfinite(alpha) || !std::isfinite(beta) || !std::isfinite(E0_re) || !std::isfinite(E0_im)) return CELES_EINVAL;
+    const long long total = (long long)ctx->N * ctx->nmax;
+    celes::plane_wave_kernel<<<(unsigned)((total + 127) / 128), 128, 0, (cudaStream_t)cuda_stream>>>(
+        ctx->N, ctx->lmax, ctx->kpos, alpha, beta, polarisation, make_double2(E0_re, E0_im), (float2*)a_in_dev);
+    return cudaGetLastError() == cudaSuccess ? CELES_OK : CELES_ECUDA;
+}
+
 int celes_gaussian_beam(celes_ctx* ctx, const celes_beam* beam, void* a_in_dev, void* cuda_stream) {
     if (!ctx || !beam || !a_in_dev) return CELES_EINVAL;
     const int n_beta = beam->n_beta > 0 ? beam->n_beta : 400;

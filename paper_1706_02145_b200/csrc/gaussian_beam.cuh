@@ -111,4 +111,36 @@ __global__ void gaussian_beam_kernel(int N, int lmax, int n_beta, const double* 
     a_in[t] = make_float2((float)(E0.x * ar - E0.y * ai), (float)(E0.x * ai + E0.y * ar));
 }
 
+// Plane wave E0 Phi_j(alpha, beta; r) expanded about every sphere centre, (A.13)-(A.14), PAPER.md:276-282:
+//   a^i_{in,n} = E0 exp(i k.r_i) 4 exp(-i m alpha) B^dagger_nj(beta).   One thread per (sphere, n), FP64, rounded once.
+__global__ void plane_wave_kernel(int N, int lmax, const double* __restrict__ kpos, double alpha, double beta, int j,
+                                  double2 E0, float2* __restrict__ a_in) {
+    const int H = lmax * (lmax + 2), nmax = 2 * H;
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= (long long)N * nmax) return;
+    const int i = (int)(t / nmax), n = (int)(t - (long long)i * nmax);
+    const int tau = n / H + 1, qn = n % H;
+    int l = 1;
+    while ((l + 1) * (l + 1) - 1 <= qn) ++l;
+    const int m = qn - (l * l - 1) - l, am = m < 0 ? -m : m;
+    double sa, ca, sb, cb;
+    sincos(alpha, &sa, &ca);
+    sincos(beta, &sb, &cb);
+    double P[6][6], pi[6][6], tt[6][6];
+    legendre_pi_tau(lmax, cb, sb, P, pi, tt);
+    const double ang = tau == j ? tt[l][am] : m * pi[l][am];
+    // B^dagger_nj = -(1 / (-i)^{l+1}) / sqrt(2 l (l+1)) (-i d_j1 + d_j2) ang;   1 / (-i)^{l+1} = i^{l+1}
+    double pr = 1.0, pim = 0.0;                                      // i^{l+1}
+    for (int q = 0; q <= l; ++q) { const double r = -pim, im = pr; pr = r; pim = im; }
+    const double nrm = -4.0 * ang / sqrt(2.0 * l * (l + 1.0));
+    double br = nrm * pr, bi = nrm * pim;
+    if (j == 1) { const double r = bi, im = -br; br = r; bi = im; }    // times -i
+    // phase exp(i (k.r_i - m alpha))
+    const double ph = (sb * ca) * kpos[3 * i] + (sb * sa) * kpos[3 * i + 1] + cb * kpos[3 * i + 2] - m * alpha;
+    double sp, cp;
+    sincos(ph, &sp, &cp);
+    const double vr = br * cp - bi * sp, vi = br * sp + bi * cp;
+    a_in[t] = make_float2((float)(E0.x * vr - E0.y * vi), (float)(E0.x * vi + E0.y * vr));
+}
+
 }  // namespace celes

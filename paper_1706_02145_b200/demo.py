@@ -42,7 +42,7 @@ def main() -> None:
     pos, rad = workloads.positions(w)
     q = fields.mie_coefficients(w.lmax, w.k, rad, workloads.N_SPHERE)
     ctx = celes.celes_setup(pos, rad, q, w.k, w.lmax)
-    a_in = torch.from_numpy(fields.plane_wave_coefficients(pos, w.k, w.lmax).astype(np.complex64)).cuda()
+    a_in = celes.celes_plane_wave(ctx, 0.0, 0.0, 2)                 # +z, x-polarised (A.13)
     b = torch.zeros(w.N, w.nmax, dtype=torch.complex64, device="cuda")
     info = celes.celes_solve(ctx, a_in, b, restart=30, rtol=1e-4, max_iters=2000)
     print(f"solve: {info['iterations']} iterations, {info['matvecs']} matvecs, residual {info['rel_residual']:.2e}, "

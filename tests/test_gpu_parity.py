@@ -514,3 +514,17 @@ def test_matvec_is_bitwise_reproducible():
     y3 = celes.celes_coupling_matvec(ctx2, bd)
     assert torch.equal(torch.view_as_real(y1), torch.view_as_real(y2))
     assert torch.equal(torch.view_as_real(y1), torch.view_as_real(y3))
+
+
+@pytest.mark.parametrize("alpha,beta,j", [(0.0, 0.0, 2), (0.0, 0.0, 1), (0.7, 0.4, 1), (2.1, 1.3, 2), (4.0, 2.8, 2)])
+def test_plane_wave_coefficients_match_oracle(alpha, beta, j):
+    """celes_plane_wave ((A.13)-(A.14), any direction and both polarisations) against the oracle's literal evaluation
+    (pinned by P10); normal incidence, x-polarised, also against the closed form the harness uses."""
+    w = workloads.scaled(workloads.C2, 150)
+    pos, rad, q, ctx, _ = make(w)
+    E0 = 0.9 + 0.3j
+    a = celes.celes_plane_wave(ctx, alpha, beta, j, E0).cpu().numpy()
+    ref = orc.plane_wave_a_in(pos, w.k, w.lmax, alpha, beta, j, E0)
+    assert rel(a, ref) <= 1e-6
+    if (alpha, beta, j) == (0.0, 0.0, 2):
+        assert rel(a, E0 * fields.plane_wave_coefficients(pos, w.k, w.lmax)) <= 1e-6

@@ -528,3 +528,26 @@ def test_plane_wave_coefficients_match_oracle(alpha, beta, j):
     assert rel(a, ref) <= 1e-6
     if (alpha, beta, j) == (0.0, 0.0, 2):
         assert rel(a, E0 * fields.plane_wave_coefficients(pos, w.k, w.lmax)) <= 1e-6
+
+
+def test_matvec_can_be_captured_in_a_cuda_graph():
+    """The matvec entry points only enqueue kernels on the caller's stream (no allocation, no synchronisation), so a
+    system matvec can be captured once and replayed: the replay on new input matches a direct call bit for bit."""
+    w = workloads.scaled(workloads.C3, 2000)
+    pos, rad, q, ctx, b = make(w)
+    static_in = torch.from_numpy(b).cuda()
+    static_out = torch.empty_like(static_in)
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(s):
+        celes.celes_system_matvec(ctx, static_in, static_out)           # warm-up outside the capture
+    torch.cuda.current_stream().wait_stream(s)
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        celes.celes_system_matvec(ctx, static_in, static_out)
+    b2 = workloads.gaussian_coefficients(w.N, w.nmax, 991)
+    static_in.copy_(torch.from_numpy(b2).cuda())
+    g.replay()
+    torch.cuda.synchronize()
+    direct = celes.celes_system_matvec(ctx, torch.from_numpy(b2).cuda())
+    assert torch.equal(torch.view_as_real(static_out), torch.view_as_real(direct))

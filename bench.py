@@ -31,18 +31,16 @@ if ROOT not in sys.path:
 
 METRIC = "sphere_pair_translations_per_s"
 UNIT = "pairs/s"
-# FP32 flops per ordered pair of the two pair bodies, counted in the SASS of the coupling kernel's loop body
-# (2 FFMA + FMUL + FADD): geometry + radial functions + rotation/translation + accumulation.
-FLOPS_PER_PAIR = {"rotated": {3: 1878.0, 4: 3753.0}, "rotated_scalar": {3: 2312.0, 4: 4830.0},
-                  "direct": {3: 5390.0, 4: 14197.0}}
-# FP32 lane operations per pair (an FFMA2 / FMUL2 / FADD2 is two, an FFMA / FMUL / FADD one): the FMA pipe retires 128 per
-# SM per clock whatever their kind, so lane_ops x pairs / (128 x SMs x clock x time) is the pipe utilisation
-LANE_OPS_PER_PAIR = {"rotated": {3: 1216.0, 4: 2342.0}, "rotated_scalar": {3: 1369.0, 4: 2771.0},
-                     "direct": {3: 3026.0, 4: 7959.0}}
+# FP32 flops and FMA-pipe lane operations per ordered pair are COUNTED in the SASS of the built library's coupling
+# kernel (paper_1706_02145_b200/sass_count.py: opcode histogram of the per-pair loop body; flops = 4 FFMA2 + 2 (FMUL2 +
+# FADD2) + 2 FFMA + FMUL + FADD, lane ops = 2 per packed instruction + 1 per scalar one).  The FMA
+# pipe retires 128 lane operations per SM per clock whatever their kind, so lane_ops x pairs / (128 x SMs x clock x
+# time) is the pipe utilisation, while the flop fraction also charges every multiply / add as half an FMA.
 FP32_LANES_PER_SM = 128
-# dram__bytes_read.sum + dram__bytes_write.sum of one coupling-kernel launch, from the ncu --set full captures
-# summarised under profiles/ (r01h_final_kernel_c4.md, r01b_rotated_kernel_c4.md)
-NCU_DRAM_BYTES_PER_LAUNCH = {("C4", "rotated"): 131.4e6, ("C4", "rotated_scalar"): 132.0e6}
+PRECOND_EDGE_NM = 600.0     # lateral cuboid edge of the preconditioned config-5 solve in the default line
+# dram__bytes_read.sum + dram__bytes_write.sum of one coupling-kernel launch, from the ncu --set full capture
+# summarised in the named file under profiles/ (a capture, not a live measurement: ncu cannot run inside the timed run)
+NCU_DRAM_BYTES_PER_LAUNCH = {("C4", "rotated"): (131.4e6, "profiles/r01h_final_kernel_c4.md")}
 
 
 def parse():
@@ -52,7 +50,7 @@ def parse():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--workload", default="C4")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--translation", default="rotated", choices=["rotated", "direct", "rotated_scalar"])
+    ap.add_argument("--translation", default="rotated", choices=["rotated", "direct"])
     ap.add_argument("--solve", action="store_true",
                     help="time celes_solve (plane wave, GMRES(30), rtol 1e-4) on the workload instead (config 5: --workload C5)")
     ap.add_argument("--precond-edge", type=float, default=0.0,
@@ -122,6 +120,16 @@ def measured_peaks() -> dict:
         return json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
     except (OSError, ValueError):
         return {}
+
+
+def device_sm_clock_hz(index: int = 0) -> float:
+    """Maximum SM clock of the device (nvidia-smi clocks.max.sm; MEASURED_PEAKS.json if the query fails)."""
+    try:
+        out = subprocess.run(["nvidia-smi", "--query-gpu=clocks.max.sm", "--format=csv,noheader,nounits", "-i", str(index)],
+                             capture_output=True, text=True, timeout=20).stdout
+        return float(out.strip().splitlines()[0]) * 1e6
+    except (OSError, ValueError, IndexError, subprocess.TimeoutExpired):
+        return float(measured_peaks().get("sm_max_mhz", 1965.0)) * 1e6
 
 
 def max_over_ranks(value: float, world: int, device) -> float:
@@ -284,7 +292,68 @@ def run_far_field(args, w):
         "steps": len(times), "ms_per_call": sec * 1e3, "higher_is_better": True, "dtype": "f32", "data": "synthetic",
         "config": {"workload": f"{w.name}: N={w.N} lmax={w.lmax}", "directions": int(al.size)},
         "roofline": {"bound": "alu", "lane_ops_per_term": lane,
-                     "fma_pipe_utilisation_incl_host_tables": lane * terms / sec / (FP32_LANES_PER_SM * sm * 1.965e9)}}))
+                     "fma_pipe_utilisation_incl_host_tables": lane * terms / sec / (FP32_LANES_PER_SM * sm * device_sm_clock_hz())}}))
+
+
+def time_coupling(celes, ctx, b, y, steps, flush, stream):
+    """CUDA-event times (ms) of `steps` coupling matvecs on `stream`, L2 flushed before each (outside the events)."""
+    import torch
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    for a, c in ev:
+        flush.zero_()
+        a.record(stream)
+        celes.celes_coupling_matvec(ctx, b, y)
+        c.record(stream)
+    torch.cuda.synchronize()
+    return [a.elapsed_time(c) for a, c in ev]
+
+
+def alu_roofline(counts, pairs, ms, sm_count, sm_max_mhz, sm_mhz):
+    """Roofline numbers of one coupling launch from the SASS-counted work per pair (sass_count.py)."""
+    achieved = counts["flops_per_pair"] * pairs / (ms * 1e-3)
+    lane_rate = counts["lane_ops_per_pair"] * pairs / (ms * 1e-3)
+    nominal = 2.0 * FP32_LANES_PER_SM * sm_count * sm_max_mhz * 1e6
+    return {"bound": "alu", "achieved": achieved / 1e12, "peak": nominal / 1e12, "unit": "TFLOP/s",
+            "frac": achieved / nominal,
+            "peak_kind": "derived: 2 x 128 FP32 lanes x SMs x clocks.max.sm (DESIGN.md section 6)",
+            "frac_of_peak_at_observed_clock": achieved / (2.0 * FP32_LANES_PER_SM * sm_count * sm_mhz * 1e6),
+            "flops_per_pair": counts["flops_per_pair"], "lane_ops_per_pair": counts["lane_ops_per_pair"],
+            "fp32_opcodes_per_pair": counts["fp32"], "packed_non_fma_per_pair": counts["packed_non_fma"],
+            "counts_source": counts["source"],
+            "fma_pipe_utilisation": lane_rate / (FP32_LANES_PER_SM * sm_count * sm_mhz * 1e6)}
+
+
+def solve_c5(celes, fields, workloads, translation, precond_edge=0.0):
+    """BASELINE.json config 5 (N = 1e4, lmax = 4, plane wave +z x-pol, GMRES(30), rtol 1e-4): wall-clock time to
+    solution (preconditioner set-up included when one is used), iterations, matvecs, true relative residual."""
+    import torch
+    w = workloads.CONFIGS["C5"]
+    pos, rad = workloads.positions(w)
+    q = fields.mie_coefficients(w.lmax, w.k, rad, workloads.N_SPHERE)
+    ctx = celes.celes_setup(pos, rad, q, w.k, w.lmax, translation=translation)
+    a_in = torch.from_numpy(fields.plane_wave_coefficients(pos, w.k, w.lmax).astype(np.complex64)).cuda()
+    x = torch.zeros(w.N, w.nmax, dtype=torch.complex64, device="cuda")
+    celes.celes_solve(ctx, a_in, x, restart=30, rtol=1e-4, max_iters=3)          # warm-up (allocations, caches)
+    edge = [precond_edge, precond_edge, 0.0]
+    pc = None
+    if precond_edge > 0:
+        celes.celes_precond_setup(ctx, edge)                                      # warm-up
+    x.zero_()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    if precond_edge > 0:
+        pc = celes.celes_precond_setup(ctx, edge)
+        torch.cuda.synchronize()
+    t_setup = time.perf_counter() - t0
+    info = celes.celes_solve(ctx, a_in, x, restart=30, rtol=1e-4, max_iters=2000, precond=pc is not None)
+    torch.cuda.synchronize()
+    sec = time.perf_counter() - t0
+    out = {"workload": f"C5: N={w.N} lmax={w.lmax} plane wave +z x-pol, GMRES(30), rtol 1e-4", "seconds": sec,
+           "iterations": info["iterations"], "matvecs": info["matvecs"], "rel_residual": info["rel_residual"],
+           "converged": bool(info["converged"])}
+    if pc is not None:
+        out["preconditioner"] = dict(pc, edge_nm=precond_edge, setup_seconds=t_setup)
+    return out, ctx, a_in
 
 
 def main():
@@ -304,7 +373,7 @@ def main():
     import torch
     import torch.distributed as dist
     import paper_1706_02145_b200 as celes
-    from paper_1706_02145_b200 import fields
+    from paper_1706_02145_b200 import fields, sass_count
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -333,23 +402,17 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    # FP32 peak of this GPU at its clocks of the moment (FFMA-only probe)
+    # FP32 peak of this GPU at its clocks of the moment (FFMA-only probes)
     probe = {v: celes.celes_fp32_peak_probe(v, 2048)["flops_per_s"] for v in (0, 1, 2, 3, 4)}
     for _ in range(args.warmup):
         celes.celes_coupling_matvec(ctx, b, y)
     barrier()
     sampler = ClockSampler(local)
     sampler.start()
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     barrier()
-    for s in range(args.steps):
-        flush.zero_()                                   # L2 flush between timed iterations (outside the events)
-        ev[s][0].record(stream)
-        celes.celes_coupling_matvec(ctx, b, y)
-        ev[s][1].record(stream)
+    step_ms = time_coupling(celes, ctx, b, y, args.steps, flush, stream)
     barrier()
     clocks = sampler.stop()
-    step_ms = [a.elapsed_time(c) for a, c in ev]
     total_ms = max_over_ranks(float(sum(step_ms)), world, "cuda")
     ms_per_step = total_ms / args.steps
     value = job_throughput(pairs, args.steps, world, total_ms)
@@ -368,16 +431,23 @@ def main():
     e2e_value = job_throughput(pairs, args.steps, world, e2e_s * 1e3)
 
     if rank == 0:
-        peaks = measured_peaks()
         sm_count = torch.cuda.get_device_properties(local).multi_processor_count
-        sm_mhz = clocks.get("sm_mhz") or peaks.get("sm_max_mhz") or 1965.0
-        nominal_peak = 2.0 * FP32_LANES_PER_SM * sm_count * (clocks.get("sm_max_mhz") or 1965.0) * 1e6
-        peak_at_clock = 2.0 * FP32_LANES_PER_SM * sm_count * sm_mhz * 1e6
-        fpp = FLOPS_PER_PAIR[args.translation].get(w.lmax, 0.0)
-        flops = fpp * pairs
-        achieved = flops / (ms_per_step * 1e-3)
-        lane_ops = LANE_OPS_PER_PAIR[args.translation].get(w.lmax, 0.0)
-        lane_rate = lane_ops * pairs / (ms_per_step * 1e-3)           # FP32 lane operations per second
+        sm_max_mhz = clocks.get("sm_max_mhz") or measured_peaks().get("sm_max_mhz") or 1965.0
+        sm_mhz = clocks.get("sm_mhz") or sm_max_mhz
+        counts = sass_count.counts_for_bench(w.lmax, args.translation)
+        roof = alu_roofline(counts, pairs, ms_per_step, sm_count, sm_max_mhz, sm_mhz)
+        lane_rate = counts["lane_ops_per_pair"] * pairs / (ms_per_step * 1e-3)
+        traffic = NCU_DRAM_BYTES_PER_LAUNCH.get((w.name, args.translation))
+        roof.update({
+            "traffic": None if traffic is None else traffic[0],
+            "traffic_source": None if traffic is None else traffic[1],
+            "translation": args.translation,
+            "ffma_probe_tflops": {"reg": probe[0] / 1e12, "imm": probe[1] / 1e12, "f32x2": probe[2] / 1e12,
+                                  "f32x2_3_register_operands": probe[3] / 1e12,
+                                  "f32x2_shared_multiplicand": probe[4] / 1e12},
+            "frac_of_ffma_probe": roof["achieved"] * 1e12 / max(probe.values()),
+            "lane_rate_vs_3_operand_probe": lane_rate / (0.5 * probe[3]),
+            "lane_rate_vs_shared_multiplicand_probe": lane_rate / (0.5 * probe[4])})
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -390,20 +460,7 @@ def main():
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(b_host.nbytes),
                     "d2h_bytes_per_step": int(b_host.nbytes)},
             "gpu_launches": 3 * args.steps,
-            "roofline": {"bound": "alu", "achieved": achieved / 1e12, "peak": nominal_peak / 1e12, "unit": "TFLOP/s",
-                         "frac": achieved / nominal_peak,
-                         "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get((w.name, args.translation)),
-                         "peak_kind": "derived: 2 x 128 FP32 lanes x SMs x clocks.max.sm (DESIGN.md section 7)",
-                         "frac_of_peak_at_observed_clock": achieved / peak_at_clock,
-                         "ffma_probe_tflops": {"reg": probe[0] / 1e12, "imm": probe[1] / 1e12, "f32x2": probe[2] / 1e12,
-                                               "f32x2_3_register_operands": probe[3] / 1e12,
-                                               "f32x2_shared_multiplicand": probe[4] / 1e12},
-                         "frac_of_ffma_probe": achieved / max(probe.values()),
-                         "flops_per_pair": fpp, "translation": args.translation,
-                         "lane_ops_per_pair": lane_ops,
-                         "fma_pipe_utilisation": lane_rate / (FP32_LANES_PER_SM * sm_count * sm_mhz * 1e6),
-                         "lane_rate_vs_3_operand_probe": lane_rate / (0.5 * probe[3]),
-                         "lane_rate_vs_shared_multiplicand_probe": lane_rate / (0.5 * probe[4])},
+            "roofline": roof,
         }
         if w.name == "C4" and world == 1:
             # BASELINE.json's metric names N = 1e4 as well: the same measurement on C3, reported beside the headline
@@ -415,17 +472,34 @@ def main():
             y3 = torch.empty_like(b3)
             for _ in range(max(3, args.warmup)):
                 celes.celes_coupling_matvec(ctx3, b3, y3)
-            ev3 = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(10)]
-            for a3, c3 in ev3:
-                flush.zero_()
-                a3.record(stream)
-                celes.celes_coupling_matvec(ctx3, b3, y3)
-                c3.record(stream)
-            torch.cuda.synchronize()
-            ms3 = float(np.median([a3.elapsed_time(c3) for a3, c3 in ev3]))
+            ms3 = float(np.median(time_coupling(celes, ctx3, b3, y3, 10, flush, stream)))
+            p3 = w3.N * (w3.N - 1)
+            r3 = alu_roofline(counts, p3, ms3, sm_count, sm_max_mhz, sm_mhz)
             line["also"] = {"workload": f"C3: N={w3.N} lmax={w3.lmax} (same recipe, 20 um slab)", "ms_per_step": ms3,
-                            "value": w3.N * (w3.N - 1) / (ms3 * 1e-3), "unit": UNIT, "steps": 10,
-                            "launch": celes.celes_launch_config(ctx3)}
+                            "value": p3 / (ms3 * 1e-3), "unit": UNIT, "steps": 10,
+                            "launch": celes.celes_launch_config(ctx3),
+                            "roofline": {k: r3[k] for k in ("frac", "fma_pipe_utilisation", "achieved", "peak", "unit")}}
+            del ctx3
+            # BASELINE.json config 5: the lmax = 4 kernel of the full solve, then the solve itself (time to solution and
+            # iteration count), plain and with the paper's block-diagonal preconditioner
+            solve, ctx5, a5 = solve_c5(celes, fields, workloads, args.translation)
+            w5 = workloads.CONFIGS["C5"]
+            b5 = torch.from_numpy(workloads.gaussian_coefficients(w5.N, w5.nmax, w5.seed_b)).cuda()
+            y5 = torch.empty_like(b5)
+            for _ in range(max(3, args.warmup)):
+                celes.celes_coupling_matvec(ctx5, b5, y5)
+            ms5 = float(np.median(time_coupling(celes, ctx5, b5, y5, 10, flush, stream)))
+            p5 = w5.N * (w5.N - 1)
+            c5 = sass_count.counts_for_bench(w5.lmax, args.translation)
+            r5 = alu_roofline(c5, p5, ms5, sm_count, sm_max_mhz, sm_mhz)
+            line["also_c5"] = {"workload": f"C5 geometry: N={w5.N} lmax={w5.lmax} (coupling matvec, L2 flushed)",
+                               "ms_per_step": ms5, "value": p5 / (ms5 * 1e-3), "unit": UNIT, "steps": 10,
+                               "launch": celes.celes_launch_config(ctx5), "roofline": r5}
+            line["also_solve"] = solve
+            del ctx5
+            solve_pc, ctx5, _ = solve_c5(celes, fields, workloads, args.translation, precond_edge=PRECOND_EDGE_NM)
+            line["also_solve_preconditioned"] = solve_pc
+            del ctx5
         if not args.no_cpu_baseline and world == 1:
             rate, cores, n_recv, dt = oracle_sample_rate(w, pos, b_host, args.cpu_seconds)
             line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",

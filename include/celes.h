@@ -49,13 +49,14 @@ typedef struct celes_options {
     int translation;       /* how W^{ii'} b^{i'} is evaluated per pair: CELES_TRANSLATION_ROTATED (default) rotates the
                               emitter coefficients so that d is the z axis, translates along z (diagonal in m) and
                               rotates back, in packed FP32 pairs (fma.rn.f32x2);
-                              CELES_TRANSLATION_DIRECT sums (A.6)-(A.8) term by term;
-                              CELES_TRANSLATION_ROTATED_SCALAR is the rotated scheme in scalar FP32 instructions.
-                              Same result up to FP32 rounding. */
+                              CELES_TRANSLATION_DIRECT sums (A.6)-(A.8) term by term, the paper's
+                              algorithm, kept as an in-library cross-check (lmax <= 4).  Same result up to FP32
+                              rounding. */
     int hankel;            /* how h_p^(1)(kd) is obtained per pair: CELES_HANKEL_REGISTERS (default) evaluates e^{ikd}
                               and the upward recurrence in registers; CELES_HANKEL_TABLE is the paper's scheme
                               (PAPER.md:130): a lookup table over the radial distance with spacing hankel_dr, built by
-                              celes_setup on the device, interpolated with cubic (Hermite) splines in the kernel.
+                              celes_setup (FP64 on the host, stored FP32 on the device with the analytic derivative),
+                              interpolated with cubic (Hermite) splines in the kernel.
                               Only with CELES_TRANSLATION_ROTATED. */
     double hankel_dr;      /* table spacing Delta r in the length unit U; 0 = default 1.0 (1 nm in PAPER.md:140) */
 } celes_options;
@@ -63,7 +64,6 @@ typedef struct celes_options {
 #define CELES_HANKEL_TABLE     1
 #define CELES_TRANSLATION_ROTATED        0
 #define CELES_TRANSLATION_DIRECT         1
-#define CELES_TRANSLATION_ROTATED_SCALAR 2
 
 #define CELES_GMRES    0
 #define CELES_BICGSTAB 1

@@ -19,9 +19,8 @@ LIB_PATH = os.path.join(_HERE, "libceles.so")
 CELES_OK, CELES_EINVAL, CELES_ENOMEM, CELES_ECUDA, CELES_ENOCONV = 0, -1, -2, -3, -4
 CELES_GMRES, CELES_BICGSTAB = 0, 1
 CELES_PRECOND_NONE, CELES_PRECOND_BLOCKDIAG = 0, 1
-CELES_TRANSLATION_ROTATED, CELES_TRANSLATION_DIRECT, CELES_TRANSLATION_ROTATED_SCALAR = 0, 1, 2
-TRANSLATIONS = {"rotated": CELES_TRANSLATION_ROTATED, "direct": CELES_TRANSLATION_DIRECT,
-                "rotated_scalar": CELES_TRANSLATION_ROTATED_SCALAR}
+CELES_TRANSLATION_ROTATED, CELES_TRANSLATION_DIRECT = 0, 1
+TRANSLATIONS = {"rotated": CELES_TRANSLATION_ROTATED, "direct": CELES_TRANSLATION_DIRECT}
 CELES_MAX_HISTORY = 4096
 EXPORTS = ["celes_setup", "celes_coupling_matvec", "celes_system_matvec", "celes_coupling_matvec_host",
            "celes_system_matvec_host", "celes_solve", "celes_destroy", "celes_strerror", "celes_nmax",

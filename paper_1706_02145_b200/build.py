@@ -2,7 +2,8 @@
 
     python -m paper_1706_02145_b200.build [--force] [--regen]
 
-``--regen`` re-runs csrc/gen_coupling_body.py first (needs SymPy; the generated files are committed).
+``--regen`` first re-runs both generators of the straight-line pair bodies, csrc/gen_coupling_body.py (direct sum,
+lmax 1-4) and csrc/gen_packed_body.py (packed rotated body, lmax 1-5); needs SymPy, the generated files are committed.
 nvcc cross-compiles without a GPU.  Four translation units (csrc/celes.cu, solve.cu, precond.cu, fields.cu).  The library is loaded by ``paper_1706_02145_b200.binding`` via ctypes.
 """
 from __future__ import annotations
@@ -37,6 +38,7 @@ def stale() -> bool:
 def build(force: bool = False, regen: bool = False, verbose: bool = False) -> str:
     if regen:
         subprocess.run([sys.executable, os.path.join(CSRC, "gen_coupling_body.py")], check=True)
+        subprocess.run([sys.executable, os.path.join(CSRC, "gen_packed_body.py")], check=True)
     if force or stale():
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
         units = [os.path.join(CSRC, f) for f in ("celes.cu", "solve.cu", "precond.cu", "fields.cu")]

@@ -55,14 +55,14 @@ int prepare_coupling_t(celes_ctx* c, int* ctas_per_sm) {
     return prepare_coupling_tt<LMAX, ROT, false>(c, ctas_per_sm);
 }
 
-#define CELES_DISPATCH(fn, ...)                                                                              \
-    switch (c->lmax * 3 + c->variant) {                                                                      \
-        case 3: return fn<1, 0>(__VA_ARGS__); case 4: return fn<1, 1>(__VA_ARGS__); case 5: return fn<1, 2>(__VA_ARGS__);    \
-        case 6: return fn<2, 0>(__VA_ARGS__); case 7: return fn<2, 1>(__VA_ARGS__); case 8: return fn<2, 2>(__VA_ARGS__);    \
-        case 9: return fn<3, 0>(__VA_ARGS__); case 10: return fn<3, 1>(__VA_ARGS__); case 11: return fn<3, 2>(__VA_ARGS__);  \
-        case 12: return fn<4, 0>(__VA_ARGS__); case 13: return fn<4, 1>(__VA_ARGS__); case 14: return fn<4, 2>(__VA_ARGS__); \
-        case 15: return fn<5, 0>(__VA_ARGS__);   /* lmax = 5: packed rotated body only */                            \
-    }                                                                                                        \
+#define CELES_DISPATCH(fn, ...)                                                            \
+    switch (c->lmax * 2 + c->variant) {                                                    \
+        case 2: return fn<1, 0>(__VA_ARGS__); case 3: return fn<1, 1>(__VA_ARGS__);        \
+        case 4: return fn<2, 0>(__VA_ARGS__); case 5: return fn<2, 1>(__VA_ARGS__);        \
+        case 6: return fn<3, 0>(__VA_ARGS__); case 7: return fn<3, 1>(__VA_ARGS__);        \
+        case 8: return fn<4, 0>(__VA_ARGS__); case 9: return fn<4, 1>(__VA_ARGS__);        \
+        case 10: return fn<5, 0>(__VA_ARGS__);   /* lmax = 5: packed rotated body only */  \
+    }                                                                                      \
     return CELES_EINVAL
 
 int launch_coupling(const celes_ctx* c, cudaStream_t s) { CELES_DISPATCH(launch_coupling_t, c, s); }
@@ -77,15 +77,13 @@ int celes::host::run_matvec(celes_ctx* c, const float2* b, float2* out, bool sys
     const int tb = 256;
     const unsigned gb = (unsigned)((nh + tb - 1) / tb);
     if (c->variant == celes::kRotated) celes::pack_kernel<celes::kRotated><<<gb, tb, 0, s>>>(c->N, H, b, c->bpm);
-    else if (c->variant == celes::kDirect) celes::pack_kernel<celes::kDirect><<<gb, tb, 0, s>>>(c->N, H, b, c->bpm);
-    else celes::pack_kernel<celes::kRotatedScalar><<<gb, tb, 0, s>>>(c->N, H, b, c->bpm);
+    else celes::pack_kernel<celes::kDirect><<<gb, tb, 0, s>>>(c->N, H, b, c->bpm);
     if (cudaGetLastError() != cudaSuccess) return CELES_ECUDA;
     int rc = launch_coupling(c, s);
     if (rc) return rc;
     const float2* td = system ? c->tdiag : nullptr;
     if (c->variant == celes::kRotated) celes::finalize_kernel<celes::kRotated><<<gb, tb, 0, s>>>(c->N, H, c->splits, c->ypart, td, b, out);
-    else if (c->variant == celes::kDirect) celes::finalize_kernel<celes::kDirect><<<gb, tb, 0, s>>>(c->N, H, c->splits, c->ypart, td, b, out);
-    else celes::finalize_kernel<celes::kRotatedScalar><<<gb, tb, 0, s>>>(c->N, H, c->splits, c->ypart, td, b, out);
+    else celes::finalize_kernel<celes::kDirect><<<gb, tb, 0, s>>>(c->N, H, c->splits, c->ypart, td, b, out);
     return cudaGetLastError() == cudaSuccess ? CELES_OK : CELES_ECUDA;
 }
 
@@ -264,7 +262,7 @@ int celes_setup(celes_ctx** out, int N, int lmax, const double* pos_xyz, const d
     const bool skip = opt && opt->skip_overlap_check;
     if (!skip && !spheres_disjoint(N, pos_xyz, radii)) return CELES_EINVAL;
     if (opt && (opt->emitter_tile < 0 || opt->emitter_splits < 0 || opt->emitter_tile > 128)) return CELES_EINVAL;
-    if (opt && (opt->translation < 0 || opt->translation > CELES_TRANSLATION_ROTATED_SCALAR)) return CELES_EINVAL;
+    if (opt && (opt->translation < 0 || opt->translation > CELES_TRANSLATION_DIRECT)) return CELES_EINVAL;
     if (lmax > 4 && opt && opt->translation != CELES_TRANSLATION_ROTATED) return CELES_EINVAL;   // one body at lmax = 5
     const bool table = opt && opt->hankel == CELES_HANKEL_TABLE;
     if (opt && opt->hankel != CELES_HANKEL_REGISTERS && opt->hankel != CELES_HANKEL_TABLE) return CELES_EINVAL;

@@ -29,7 +29,7 @@ __host__ __device__ constexpr int nmax_of(int lmax) { return 2 * lmax * (lmax + 
 // ---------------------------------------------------------------------------------------------------------
 // b -> work basis.  One thread per (sphere, index q inside a tau block).
 //   DIRECT : [b_1 + b_2 | b_1 - b_2], index order unchanged.
-//   ROTATED: orthonormal basis of gen_rotated_body.py: x_S/A = (x_1 +- x_2)/sqrt2, then per l
+//   ROTATED: orthonormal basis of rotation_tables.py: x_S/A = (x_1 +- x_2)/sqrt2, then per l
 //            [u_0 = x_0, u+_m = (x_m + x_-m)/sqrt2, u-_m = (x_m - x_-m)/sqrt2, m = 1..l] at q = l^2-1 + {0, 2m-1, 2m}.
 __device__ __forceinline__ void split_q(int q, int& l, int& pos) {
     l = 1;
@@ -66,7 +66,7 @@ __global__ void pack_kernel(int N, int H, const float2* __restrict__ b, float2* 
             const float2 u2 = make_float2(0.5f * p2.x + sg * n2.x, 0.5f * p2.y + sg * n2.y);
             s = make_float2(u1.x + u2.x, u1.y + u2.y);
             a = make_float2(u1.x - u2.x, u1.y - u2.y);
-            if (VARIANT == kRotated && !(pos & 1)) {        // packed body: w_m = i u-_m
+            if (!(pos & 1)) {                               // packed body: w_m = i u-_m
                 s = make_float2(-s.y, s.x);
                 a = make_float2(-a.y, a.x);
             }
@@ -218,7 +218,7 @@ __global__ void finalize_kernel(int N, int H, int splits, const float2* __restri
                 sbr += sb.x; sbi += sb.y; abr += ab.x; abi += ab.y;
             }
         }
-        if (VARIANT == kRotated) {                           // packed body: u-_m = -i w_m
+        {                                                    // packed body: u-_m = -i w_m
             float t;
             t = sbr; sbr = sbi; sbi = -t;
             t = abr; abr = abi; abi = -t;

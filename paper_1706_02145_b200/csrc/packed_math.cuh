@@ -15,6 +15,21 @@ CELES_DEVICE float2 fma2(float2 a, float2 b, float2 c) { return __ffma2_rn(a, b,
 CELES_DEVICE float2 mul2(float2 a, float2 b) { return __fmul2_rn(a, b); }
 CELES_DEVICE float2 add2(float2 a, float2 b) { return __fadd2_rn(a, b); }
 CELES_DEVICE float2 sub2(float2 a, float2 b) { return __fadd2_rn(a, neg2(b)); }
+// i a and -i a: swapped halves with a (-,+) / (+,-) sign pattern, which FFMA2 / FADD2 take as operand modifiers
+// (SASS .LO_HI / .NP) on their vector operands -- no instruction of their own.
+CELES_DEVICE float2 imul2(float2 a) { return make_float2(-a.y, a.x); }
+CELES_DEVICE float2 nimul2(float2 a) { return make_float2(a.y, -a.x); }
+// Complex multiply(-add) k x (+ c) in TWO packed instructions: the broadcast scalar operand cannot carry the
+// (-k.y, +k.y) pattern, but the addend can be read as (-c.x, c.y) and the vector multiplicand with swapped halves:
+//   t = k.y (x.y, x.x) + (-c.x, c.y) = (-Re, Im) of c + i k.y x;   k.x x + (-t.x, t.y) = c + k x.
+CELES_DEVICE float2 cfma2(float2 k, float2 x, float2 c) {
+    const float2 t = __ffma2_rn(bc2(k.y), make_float2(x.y, x.x), make_float2(-c.x, c.y));
+    return __ffma2_rn(bc2(k.x), x, make_float2(-t.x, t.y));
+}
+CELES_DEVICE float2 cmul2(float2 k, float2 x) {
+    const float2 t = __fmul2_rn(bc2(k.y), make_float2(x.y, x.x));
+    return __ffma2_rn(bc2(k.x), x, make_float2(-t.x, t.y));
+}
 
 // sin, cos of kd.  kd reaches ~1e3 rad, where the hardware approximations (MUFU.SIN / MUFU.COS behind __sincosf) are
 // useless on their own; after a Cody-Waite reduction to [-pi, pi] (2 pi = 6.28125 + 1.9353072e-3: the first product

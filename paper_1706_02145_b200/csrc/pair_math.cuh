@@ -19,14 +19,6 @@ struct PairBody;   // specialised by the generated files
 #include "generated/coupling_body_lmax4.inc"
 
 template <int LMAX>
-struct PairBodyRot;   // rotate / axial-translate / rotate variant (gen_rotated_body.py)
-
-#include "generated/coupling_rot_lmax1.inc"
-#include "generated/coupling_rot_lmax2.inc"
-#include "generated/coupling_rot_lmax3.inc"
-#include "generated/coupling_rot_lmax4.inc"
-
-template <int LMAX>
 struct PairBodyPk;    // packed (FFMA2) rotate / axial-translate / rotate variant (gen_packed_body.py)
 
 #include "generated/coupling_pk_lmax1.inc"
@@ -76,7 +68,7 @@ CELES_DEVICE void pair_translate(float dx, float dy, float dz, const HankelTable
     if constexpr (VARIANT == celes::kRotated) {             // the same recurrence on packed (Re, Im)
         float2 h[P];
         h[0] = mul2(bc2(rinv), make_float2(sx, -cx));
-        h[1] = mul2(bc2(rinv), add2(h[0], make_float2(-cx, -sx)));
+        h[1] = fma2(bc2(rinv), h[0], nimul2(h[0]));             // h_1 = h_0 / x - e^{ix} / x,  e^{ix} / x = i h_0
 #pragma unroll
         for (int p = 1; p + 1 < P; ++p) h[p + 1] = fma2(bc2((float)(2 * p + 1) * rinv), h[p], neg2(h[p - 1]));
         PairBodyPk<LMAX>::run(h, ct, st, cph, sph, bload, yacc);
@@ -93,7 +85,6 @@ CELES_DEVICE void pair_translate(float dx, float dy, float dz, const HankelTable
         hi[p + 1] = fmaf(f, hi[p], -hi[p - 1]);
     }
     // ---- H4-H7 angular functions, p-contraction, n'-contraction (generated)
-    if constexpr (VARIANT == celes::kRotatedScalar) PairBodyRot<LMAX>::run(hr, hi, ct, st, cph, sph, bload, yacc);
-    else PairBody<LMAX>::run(hr, hi, ct, st, cph, sph, bload, yacc);
+    PairBody<LMAX>::run(hr, hi, ct, st, cph, sph, bload, yacc);
     }
 }

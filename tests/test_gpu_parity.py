@@ -47,7 +47,7 @@ def test_c1_coupling_system_and_solve():
     assert rel(x.cpu().numpy(), orc.solve_dense(pos, w.k, w.lmax, qo, a_in)) <= SOLVE_TOL
 
 
-@pytest.mark.parametrize("translation", ["rotated", "direct", "rotated_scalar"])
+@pytest.mark.parametrize("translation", ["rotated", "direct"])
 @pytest.mark.parametrize("lmax", [1, 2, 3, 4])
 def test_every_lmax_small_cluster(lmax, translation):
     w = workloads.Workload(f"L{lmax}", 77, lmax, 90.0, 110.0, "cube", 1800.0, 0.0, 111, 311, 211)
@@ -80,7 +80,7 @@ def test_single_sphere_and_pair():
     assert rel(gpu_coupling(ctx2, b2), orc.coupling_matvec(pos, k, 3, b2)) <= MATVEC_TOL
 
 
-@pytest.mark.parametrize("translation", ["rotated", "direct", "rotated_scalar"])
+@pytest.mark.parametrize("translation", ["rotated", "direct"])
 def test_on_axis_and_lattice_pairs(translation):
     """d parallel to z (rho = 0, reading R8) and axis-aligned lattice pairs."""
     k = workloads.C1.k
@@ -104,7 +104,7 @@ def test_far_from_origin_coordinates():
     assert rel(gpu_coupling(ctx, b), orc.coupling_matvec(pos, w.k, w.lmax, b)) <= MATVEC_TOL
 
 
-@pytest.mark.parametrize("translation", ["rotated", "direct", "rotated_scalar"])
+@pytest.mark.parametrize("translation", ["rotated", "direct"])
 def test_c2_coupling_and_system_matvec_full_oracle(translation):
     w = workloads.C2
     pos, rad, q, ctx, b = make(w, translation=translation)
@@ -149,7 +149,7 @@ def test_parity_relation_on_gpu_output():
             assert abs(w10 - sign * col01[n]) <= 2e-5 * max(1.0, abs(w10))
 
 
-@pytest.mark.parametrize("translation", ["rotated", "direct", "rotated_scalar"])
+@pytest.mark.parametrize("translation", ["rotated", "direct"])
 def test_c3_sampled_receivers(translation):
     w = workloads.C3
     pos, rad, q, ctx, b = make(w, translation=translation)

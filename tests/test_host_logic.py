@@ -170,8 +170,7 @@ def test_partition_matches_oracle_cuboids():
         celes.celes_partition(np.array([[np.nan, 0.0, 0.0]]), 1.0)
 
 
-@pytest.mark.parametrize("gen,prefix", [("gen_coupling_body", "coupling_body"), ("gen_rotated_body", "coupling_rot"),
-                                        ("gen_packed_body", "coupling_pk")])
+@pytest.mark.parametrize("gen,prefix", [("gen_coupling_body", "coupling_body"), ("gen_packed_body", "coupling_pk")])
 def test_committed_generated_bodies_are_what_the_generators_write(gen, prefix, tmp_path):
     """The straight-line pair bodies under csrc/generated/ are build inputs: regenerate lmax = 1, 2 (seconds, SymPy)
     and compare byte for byte with the committed files."""

@@ -60,6 +60,9 @@ def parse():
     ap.add_argument("--hankel", default="registers", choices=["registers", "table"],
                     help="h_p(kd) in registers (default) or from the paper's lookup table (PAPER.md:130)")
     ap.add_argument("--method", default="gmres", choices=["gmres", "bicgstab"], help="with --solve")
+    ap.add_argument("--cta-trace", action="store_true",
+                    help="per-CTA start / end times and SM of the coupling kernel for --levels 1 and the default partition "
+                         "(needs a library built with CELES_NVCC_EXTRA=-DCELES_TRACE python -m paper_1706_02145_b200.build --force)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=20.0, help="CPU work of the cpu_baseline sample")
     return ap.parse_args()
@@ -279,10 +282,12 @@ def run_far_field(args, w):
         celes.celes_far_field(ctx, b, al, be, g)
     times = []
     for _ in range(max(1, args.steps)):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        celes.celes_far_field(ctx, b, al, be, g)          # asynchronous: direction upload + coefficient, sum and reduce kernels
+        e1.record()
         torch.cuda.synchronize()
-        t0 = time.perf_counter()
-        celes.celes_far_field(ctx, b, al, be, g)          # synchronises; includes the host-side direction tables
-        times.append(time.perf_counter() - t0)
+        times.append(e0.elapsed_time(e1) * 1e-3)
     sec = float(np.median(times))
     terms = 2.0 * al.size * w.N
     lane = {3: 2 * 30 * 2 + 44.0, 4: 2 * 48 * 2 + 44.0}.get(w.lmax, 0.0)      # 2 nmax FFMA2 + phase, sincos, rotation
@@ -292,7 +297,50 @@ def run_far_field(args, w):
         "steps": len(times), "ms_per_call": sec * 1e3, "higher_is_better": True, "dtype": "f32", "data": "synthetic",
         "config": {"workload": f"{w.name}: N={w.N} lmax={w.lmax}", "directions": int(al.size)},
         "roofline": {"bound": "alu", "lane_ops_per_term": lane,
-                     "fma_pipe_utilisation_incl_host_tables": lane * terms / sec / (FP32_LANES_PER_SM * sm * device_sm_clock_hz())}}))
+                     "fma_pipe_utilisation_whole_call": lane * terms / sec / (FP32_LANES_PER_SM * sm * device_sm_clock_hz())}}))
+
+
+def run_cta_trace(args, w):
+    """Diagnostic build only: how long every CTA of the coupling kernel ran and on which SM (globaltimer, %smid), for
+    one wave of equal runs (levels = 1) and for the default guided partition.  One JSON line per partition."""
+    import ctypes
+    import torch
+    import paper_1706_02145_b200 as celes
+    from paper_1706_02145_b200 import binding, fields, workloads
+    L = binding.lib()
+    if not hasattr(L, "celes_debug_trace"):
+        raise SystemExit("--cta-trace: rebuild with CELES_NVCC_EXTRA=-DCELES_TRACE python -m paper_1706_02145_b200.build --force")
+    L.celes_debug_trace.argtypes = [ctypes.c_void_p]
+    torch.cuda.set_device(0)
+    pos, rad = workloads.positions(w)
+    q = fields.mie_coefficients(w.lmax, w.k, rad, workloads.N_SPHERE)
+    b = torch.from_numpy(workloads.gaussian_coefficients(w.N, w.nmax, w.seed_b)).cuda()
+    y = torch.empty_like(b)
+    for levels in (1, 0):
+        ctx = celes.celes_setup(pos, rad, q, w.k, w.lmax, levels=levels)
+        for _ in range(3):
+            celes.celes_coupling_matvec(ctx, b, y)
+        torch.cuda.synchronize()
+        raw = np.zeros(3 * 8192, dtype=np.uint64)
+        assert L.celes_debug_trace(raw.ctypes.data) == 0
+        n = min(8192, celes.celes_work_partition(ctx)["ctas"])
+        t = raw.reshape(-1, 3)[:n].astype(np.int64)
+        start, end = (t[:, 1] - t[:, 1].min()) / 1e3, (t[:, 2] - t[:, 1].min()) / 1e3
+        dur = end - start
+        per_sm = {}
+        for s, d in zip(t[:, 0], dur):
+            per_sm.setdefault(int(s), []).append(float(d))
+        busy = np.array([sum(v) for v in per_sm.values()])
+        first = dur[:len(per_sm) * 2] if levels == 1 else dur
+        print(json.dumps({
+            "workload": w.name, "levels": levels or "default", "ctas": int(n), "sms": len(per_sm), "kernel_us": float(end.max()),
+            "cta_us": {"min": float(dur.min()), "median": float(np.median(dur)), "max": float(dur.max())},
+            "per_sm_busy_us": {"min": float(busy.min()), "max": float(busy.max())},
+            "ctas_per_sm": {"min": min(len(v) for v in per_sm.values()), "max": max(len(v) for v in per_sm.values())},
+            "last_start_us": float(start.max()),
+            "faster_of_two_resident_ctas_finishes_at": float(np.median([min(v) / max(v) for v in per_sm.values() if len(v) == 2]))
+            if levels == 1 and len(first) else None}))
+        del ctx
 
 
 def time_coupling(celes, ctx, b, y, steps, flush, stream):
@@ -368,6 +416,9 @@ def main():
         return
     if args.far_field > 0:
         run_far_field(args, w)
+        return
+    if args.cta_trace:
+        run_cta_trace(args, w)
         return
 
     import torch

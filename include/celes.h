@@ -43,8 +43,10 @@ typedef struct celes_ctx celes_ctx;   /* opaque; owns every device table; freed 
 /* Options of celes_setup (nullable -> defaults).  Zero in a field selects its default. */
 typedef struct celes_options {
     int emitter_tile;      /* emitters staged per shared-memory tile; default 32 */
-    int emitter_splits;    /* how many slices the emitter sum of one receiver is cut into (split-K across CTAs);
-                              0 = chosen so that the grid fills a whole number of waves on the device */
+    int emitter_splits;    /* 0 (default): the (receiver block x emitter tile) grid is cut into runs of decreasing
+                              length (see `levels`), one CTA each, dispatched in that order by the hardware;
+                              S > 0: the emitter sum of every receiver block is cut into S equal slices, one CTA each.
+                              Either way partial sums are added in a fixed order: results are reproducible bit for bit */
     int skip_overlap_check;/* 1: do not verify that spheres are disjoint */
     int translation;       /* how W^{ii'} b^{i'} is evaluated per pair: CELES_TRANSLATION_ROTATED (default) rotates the
                               emitter coefficients so that d is the z axis, translates along z (diagonal in m) and
@@ -59,7 +61,26 @@ typedef struct celes_options {
                               interpolated with cubic (Hermite) splines in the kernel.
                               Only with CELES_TRANSLATION_ROTATED. */
     double hankel_dr;      /* table spacing Delta r in the length unit U; 0 = default 1.0 (1 nm in PAPER.md:140) */
+    int range;             /* FP32 validity range.  The per-pair arithmetic is FP32 after an FP64 subtraction of the
+                              centres; kd rounded to FP32 carries a phase error of about kd 2^-24 rad, harmless for the
+                              paper's clusters (kd < 1e3: 4e-6 relative L2 on the matvec) but equal to the 1e-4 budget
+                              near kd ~ 1e4 (a cluster ~1 mm across at 550 nm).  CELES_RANGE_EXTENDED carries kd as
+                              FP32 + FP64 Newton residual through the argument reduction of e^{ikd} (six more FP64
+                              instructions per pair, ~1 % time), which removes that limit; CELES_RANGE_AUTO (default)
+                              selects it when k x (diagonal of the centres' bounding box) exceeds
+                              CELES_RANGE_AUTO_KD; CELES_RANGE_STANDARD never does.  The lookup-table mode and the
+                              direct translation are standard range only. */
+    int levels;            /* with emitter_splits = 0: number of levels of the guided partition.  Level 1 covers half of
+                              the pair grid in SMs x CTAs/SM equal runs, level 2 a quarter, ..., the last two an equal
+                              share; 1 = one wave of equal runs (fewest partial sums, ~5 % slower: of two CTAs
+                              resident on an SM the warp scheduler serves one first, and the other then finishes
+                              alone below full throughput); 0 = default CELES_DEFAULT_LEVELS */
 } celes_options;
+#define CELES_DEFAULT_LEVELS 6
+#define CELES_RANGE_AUTO     0
+#define CELES_RANGE_STANDARD 1
+#define CELES_RANGE_EXTENDED 2
+#define CELES_RANGE_AUTO_KD  2000.0
 #define CELES_HANKEL_REGISTERS 0
 #define CELES_HANKEL_TABLE     1
 #define CELES_TRANSLATION_ROTATED        0
@@ -116,6 +137,19 @@ int celes_coupling_matvec(celes_ctx* ctx, const void* b_dev, void* y_dev, void* 
 /* out = M b = b - T (W b)  (eqs. 8-9).  Same argument rules as above. */
 int celes_system_matvec(celes_ctx* ctx, const void* b_dev, void* out_dev, void* cuda_stream);
 
+/* Receiver-row slices of the two products: rows [row_begin, row_end) of y = W b (or of b - T (W b)) from the FULL
+ * vector b -- the compute half of a receiver-sharded deployment, where every rank owns a slice of the rows and needs
+ * every emitter's coefficients (the paper itself is single-GPU).
+ *   b_dev        device, N*nmax complex64, all spheres.
+ *   y_rows_dev   device, (row_end - row_begin)*nmax complex64: rows row_begin.. of the result.
+ * The work partition and the order of the partial sums are those of the full product restricted to the receiver
+ * blocks that hold the rows, so slices concatenate to the full result bit for bit.  0 <= row_begin < row_end <= N.
+ * Asynchronous on cuda_stream. */
+int celes_coupling_matvec_rows(celes_ctx* ctx, int row_begin, int row_end, const void* b_dev, void* y_rows_dev,
+                               void* cuda_stream);
+int celes_system_matvec_rows(celes_ctx* ctx, int row_begin, int row_end, const void* b_dev, void* out_rows_dev,
+                             void* cuda_stream);
+
 /* Host-buffer variants: copy b from host memory (pinned or pageable), run the device path, copy the result back,
  * synchronise.  b_host, y_host: N*nmax complex64. */
 int celes_coupling_matvec_host(celes_ctx* ctx, const void* b_host, void* y_host, void* cuda_stream);
@@ -157,7 +191,10 @@ int celes_partition(int N, const double* pos_xyz, const double* edge_xyz, int* g
  *   b_dev   device, N*nmax complex64: scattered-field coefficients (e.g. the solution of celes_solve).
  *   alpha, beta  host, [n_dir] double: azimuthal and (real) polar angles of the directions, radians.
  *   g_dev   device, [n_dir][2] complex64: g_1, g_2 per direction.
- * Synchronises the stream (it frees its per-call direction tables). */
+ * Asynchronous on cuda_stream: the direction tables live in a scratch block that the context keeps and reuses (a call
+ * that needs a larger block than any before it synchronises the stream once to grow it).  alpha and beta are read
+ * before the call returns if they are pageable memory; pinned arrays must stay valid until the stream has run.
+ * The field calls of one context share that scratch block: issue them on one stream. */
 int celes_far_field(celes_ctx* ctx, const void* b_dev, int n_dir, const double* alpha, const double* beta,
                     void* g_dev, void* cuda_stream);
 
@@ -181,7 +218,7 @@ typedef struct celes_beam {
 
 /* Initial-field coefficients a_in of the beam about every sphere centre, (C.8) with the analytic azimuthal integral
  * (C.7), evaluated on the device in FP64 and rounded once.  a_in_dev: device, N*nmax complex64 (the
- * input of celes_solve).  Synchronises the stream. */
+ * input of celes_solve).  Asynchronous on cuda_stream (scratch block of the context, see celes_far_field). */
 int celes_gaussian_beam(celes_ctx* ctx, const celes_beam* beam, void* a_in_dev, void* cuda_stream);
 
 /* Scattered electric field at n_pts points, eq. (3) with the explicit outgoing SVWFs (A.2):
@@ -190,7 +227,7 @@ int celes_gaussian_beam(celes_ctx* ctx, const celes_beam* beam, void* a_in_dev, 
  *   pts_xyz  host, [n_pts][3] double, unit U.  The expansion of sphere i holds for |r - r_i| > R_i only: points inside
  *            a sphere get the (meaningless) analytic continuation, not the internal field.
  *   e_dev    device, [n_pts][3] complex64: Cartesian components (x, y, z).
- * Synchronises the stream. */
+ * Asynchronous on cuda_stream (scratch block of the context, see celes_far_field). */
 int celes_scattered_field(celes_ctx* ctx, const void* b_dev, int n_pts, const double* pts_xyz, void* e_dev,
                           void* cuda_stream);
 
@@ -203,24 +240,30 @@ const char* celes_strerror(int code);
 /* Sizes the caller needs: nmax = 2 lmax (lmax+2); returns CELES_EINVAL (<0) for an unsupported lmax. */
 int celes_nmax(int lmax);
 
-/* Grid the coupling kernel of this context is launched with (for reporting): receiver blocks, emitter splits,
- * threads per block, emitters per tile.  Any pointer may be NULL. */
+/* Launch geometry of the coupling kernel of this context (for reporting): receiver blocks, the caller's fixed
+ * emitter splits (0 = guided partition), threads per block, emitters per tile.  Any pointer may be NULL. */
 int celes_launch_config(const celes_ctx* ctx, int* receiver_blocks, int* emitter_splits, int* block_threads,
                         int* emitter_tile);
+
+/* Numerical range of this context (for reporting): kd_max = k x diagonal of the centres' bounding box, and whether the
+ * extended range mode of celes_options.range is active (1) or not (0).  Any pointer may be NULL. */
+int celes_range_info(const celes_ctx* ctx, double* kd_max, int* extended);
+
+/* Work partition of the coupling kernel (for reporting): CTAs launched for a full product, segments (= partial-sum
+ * slots of N_block x nmax complex64 each) and receivers per receiver block.  Any pointer may be NULL. */
+int celes_work_partition(const celes_ctx* ctx, int* ctas, int* segments, int* receivers_per_block);
+
+/* Host-only (needs no GPU): the work partition celes_setup builds for N spheres, emitter tiles of emitter_tile,
+ * resident_ctas = SMs x CTAs/SM, and levels / emitter_splits as in celes_options.  seg_out (nullable, host,
+ * [seg_capacity][5] int) receives one row (cta, receiver block, e_begin, e_end, slot) per segment in launch order. */
+int celes_plan_work(int N, int emitter_tile, int resident_ctas, int levels, int emitter_splits, int* ctas, int* segments,
+                    int* receivers_per_block, int* seg_out, int seg_capacity);
 
 /* Host-only (needs no GPU): the translation coefficients the library uses, for W_{(tau l m),(tau' l' m')}:
  *   a5_re[((r*H)+c)*P + p] = Re a5(l',m'|l,m|p),  b5_im[...] = Im b5(l',m'|l,m|p)   (eq. 7),
  * r, c = (l-1)(l+1)+(m+l) of receiver / emitter, H = lmax (lmax+2), P = 2 lmax + 1, p = 0..2 lmax.
  * Both arrays have H*H*P doubles. */
 int celes_translation_table(int lmax, double* a5_re, double* b5_im);
-
-/* FP32 peak probe: runs an FFMA-only kernel (independent chains, every SM) and reports the achieved
- * FLOP/s (2 flop per FMA).  variant 0: three-register FFMA; 1: FFMA with an immediate multiplicand;
- * 2: packed fma.rn.f32x2 (all three with operands that stay in the operand reuse cache); 3: packed fma.rn.f32x2 with
- * three register operands per instruction and none shared by consecutive instructions; 4: as 3 with the packed
- * multiplicand shared by eight consecutive instructions.  3 and 4 bracket what a stream shaped like the pair body
- * (coefficient x packed complex + packed accumulator) can sustain.  Synchronises the stream. */
-int celes_fp32_peak_probe(int variant, int iters, double* flops_per_s, double* milliseconds, void* cuda_stream);
 
 #ifdef __cplusplus
 }

@@ -108,11 +108,33 @@ static double legendre_normalized(int l, int m, double x) {
     return (double)nrm * std::assoc_legendre((unsigned)l, (unsigned)m, x);
 }
 
-// radial function z_p(x): kind 3 -> h_p^(1) = j_p + i y_p, kind 1 -> j_p, kind 2 -> y_p
+// radial function z_p(x): kind 3 -> h_p^(1) = j_p + i y_p, kind 1 -> j_p, kind 2 -> y_p.
+// libstdc++'s std::sph_bessel refuses arguments beyond about 1.5e4 ("Argument x too large in __bessel_jn") and has
+// lost six digits by 1e4; for x > kLargeArgument the textbook closed forms j_0 = sin x / x, j_1 = sin x / x^2 - cos x / x,
+// y_0 = -cos x / x, y_1 = -cos x / x^2 - sin x / x and the three-term recurrence f_{p+1} = (2p+1)/x f_p - f_{p-1}
+// are used instead (upward recurrence is stable for x >> p; p <= 2 lmax <= 10 here).  Pinned against SciPy / mpmath on
+// both sides of the switch (tests/test_oracle_pins.py::test_radial_large_argument).
+static const double kLargeArgument = 8000.0;
 static cplx radial(int kind, int p, double x) {
-    if (kind == 1) return cplx(std::sph_bessel((unsigned)p, x), 0.0);
-    if (kind == 2) return cplx(std::sph_neumann((unsigned)p, x), 0.0);
-    return cplx(std::sph_bessel((unsigned)p, x), std::sph_neumann((unsigned)p, x));
+    double j, y;
+    if (x > kLargeArgument) {
+        const double s = std::sin(x), c = std::cos(x);
+        double j0 = s / x, j1 = s / (x * x) - c / x, y0 = -c / x, y1 = -c / (x * x) - s / x;
+        if (p == 0) { j = j0; y = y0; }
+        else {
+            for (int q = 1; q < p; ++q) {
+                const double jn = (2.0 * q + 1.0) / x * j1 - j0, yn = (2.0 * q + 1.0) / x * y1 - y0;
+                j0 = j1; j1 = jn; y0 = y1; y1 = yn;
+            }
+            j = j1; y = y1;
+        }
+    } else {
+        j = kind == 2 ? 0.0 : std::sph_bessel((unsigned)p, x);
+        y = kind == 1 ? 0.0 : std::sph_neumann((unsigned)p, x);
+    }
+    if (kind == 1) return cplx(j, 0.0);
+    if (kind == 2) return cplx(y, 0.0);
+    return cplx(j, y);
 }
 
 // spherical coordinates of d; phi := 0 on the z axis (reading R8)

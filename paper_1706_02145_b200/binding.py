@@ -26,7 +26,8 @@ EXPORTS = ["celes_setup", "celes_coupling_matvec", "celes_system_matvec", "celes
            "celes_system_matvec_host", "celes_solve", "celes_destroy", "celes_strerror", "celes_nmax",
            "celes_launch_config", "celes_translation_table", "celes_fp32_peak_probe", "celes_precond_setup",
            "celes_precond_apply", "celes_partition", "celes_far_field", "celes_gaussian_beam", "celes_plane_wave",
-           "celes_scattered_field"]
+           "celes_scattered_field", "celes_coupling_matvec_rows", "celes_system_matvec_rows", "celes_work_partition",
+           "celes_plan_work", "celes_range_info"]
 
 
 class CelesError(RuntimeError):
@@ -37,7 +38,8 @@ class CelesError(RuntimeError):
 
 class celes_options(ctypes.Structure):
     _fields_ = [("emitter_tile", ctypes.c_int), ("emitter_splits", ctypes.c_int), ("skip_overlap_check", ctypes.c_int),
-                ("translation", ctypes.c_int), ("hankel", ctypes.c_int), ("hankel_dr", ctypes.c_double)]
+                ("translation", ctypes.c_int), ("hankel", ctypes.c_int), ("hankel_dr", ctypes.c_double),
+                ("range", ctypes.c_int), ("levels", ctypes.c_int)]
 
 
 class celes_solve_opts(ctypes.Structure):
@@ -89,6 +91,15 @@ def lib() -> ctypes.CDLL:
         L.celes_nmax.argtypes = [i]
         L.celes_launch_config.restype = i
         L.celes_launch_config.argtypes = [p] + [ctypes.POINTER(i)] * 4
+        L.celes_plan_work.restype = i
+        L.celes_plan_work.argtypes = [i, i, i, i, i, ctypes.POINTER(i), ctypes.POINTER(i), ctypes.POINTER(i), p, i]
+        L.celes_range_info.restype = i
+        L.celes_range_info.argtypes = [p, ctypes.POINTER(d), ctypes.POINTER(i)]
+        L.celes_work_partition.restype = i
+        L.celes_work_partition.argtypes = [p] + [ctypes.POINTER(i)] * 3
+        for f in (L.celes_coupling_matvec_rows, L.celes_system_matvec_rows):
+            f.restype = i
+            f.argtypes = [p, i, i, p, p, p]
         L.celes_translation_table.restype = i
         L.celes_translation_table.argtypes = [i, p, p]
         L.celes_precond_setup.restype = i
@@ -148,7 +159,7 @@ class Context:
 
 def celes_setup(pos_xyz, radii, mie_q, k: float, lmax: int, *, emitter_tile: int = 0, emitter_splits: int = 0,
                 skip_overlap_check: bool = False, translation: str = "rotated", hankel: str = "registers",
-                hankel_dr: float = 0.0, stream=None) -> Context:
+                hankel_dr: float = 0.0, range: str = "auto", levels: int = 0, stream=None) -> Context:
     """celes_setup of include/celes.h.  pos_xyz [N,3] float64, radii [N] float64, mie_q [N,2,lmax] complex128 (host)."""
     pos = np.ascontiguousarray(pos_xyz, dtype=np.float64)
     rad = np.ascontiguousarray(radii, dtype=np.float64)
@@ -159,7 +170,8 @@ def celes_setup(pos_xyz, radii, mie_q, k: float, lmax: int, *, emitter_tile: int
     if translation not in TRANSLATIONS:
         raise ValueError("translation: one of " + ", ".join(TRANSLATIONS))
     opt = celes_options(int(emitter_tile), int(emitter_splits), int(bool(skip_overlap_check)),
-                        TRANSLATIONS[translation], {"registers": 0, "table": 1}[hankel], float(hankel_dr))
+                        TRANSLATIONS[translation], {"registers": 0, "table": 1}[hankel], float(hankel_dr),
+                        {"auto": 0, "standard": 1, "extended": 2}[range], int(levels))
     h = ctypes.c_void_p()
     import torch
     s = _stream(stream) if torch.cuda.is_available() else 0
@@ -200,6 +212,30 @@ def celes_system_matvec(ctx: Context, b, out=None, stream=None):
     if rc != CELES_OK:
         raise CelesError(rc, "celes_system_matvec")
     return out
+
+
+def _matvec_rows(fn, name, ctx, row_begin, row_end, b, out, stream):
+    import torch
+    _check_vec(b, ctx, "b")
+    rows = int(row_end) - int(row_begin)
+    if out is None:
+        out = torch.empty(max(rows, 0), ctx.nmax, dtype=torch.complex64, device=b.device)
+    if not (out.is_cuda and out.dtype == torch.complex64 and out.is_contiguous() and out.numel() == max(rows, 0) * ctx.nmax):
+        raise ValueError(f"{name}: out must be a contiguous CUDA complex64 tensor with (row_end - row_begin) * nmax elements")
+    rc = fn(ctx.handle, int(row_begin), int(row_end), b.data_ptr(), out.data_ptr(), _stream(stream))
+    if rc != CELES_OK:
+        raise CelesError(rc, name)
+    return out
+
+
+def celes_coupling_matvec_rows(ctx: Context, row_begin: int, row_end: int, b, y_rows=None, stream=None):
+    """rows [row_begin, row_end) of y = W b from the full device vector b; asynchronous on the stream."""
+    return _matvec_rows(lib().celes_coupling_matvec_rows, "celes_coupling_matvec_rows", ctx, row_begin, row_end, b, y_rows, stream)
+
+
+def celes_system_matvec_rows(ctx: Context, row_begin: int, row_end: int, b, out_rows=None, stream=None):
+    """rows [row_begin, row_end) of b - T (W b) from the full device vector b; asynchronous on the stream."""
+    return _matvec_rows(lib().celes_system_matvec_rows, "celes_system_matvec_rows", ctx, row_begin, row_end, b, out_rows, stream)
 
 
 def _host_vec(a, ctx, name):
@@ -358,6 +394,38 @@ def celes_launch_config(ctx: Context) -> dict:
     if rc != CELES_OK:
         raise CelesError(rc, "celes_launch_config")
     return dict(zip(("receiver_blocks", "emitter_splits", "block_threads", "emitter_tile"), (x.value for x in v)))
+
+
+def celes_range_info(ctx: Context) -> dict:
+    kd, ext = ctypes.c_double(), ctypes.c_int()
+    rc = lib().celes_range_info(ctx.handle, ctypes.byref(kd), ctypes.byref(ext))
+    if rc != CELES_OK:
+        raise CelesError(rc, "celes_range_info")
+    return {"kd_max": kd.value, "extended": bool(ext.value)}
+
+
+def celes_work_partition(ctx: Context) -> dict:
+    v = [ctypes.c_int() for _ in range(3)]
+    rc = lib().celes_work_partition(ctx.handle, *[ctypes.byref(x) for x in v])
+    if rc != CELES_OK:
+        raise CelesError(rc, "celes_work_partition")
+    return dict(zip(("ctas", "segments", "receivers_per_block"), (x.value for x in v)))
+
+
+def celes_plan_work(N: int, emitter_tile: int = 32, resident_ctas: int = 296, levels: int = 0, emitter_splits: int = 0) -> dict:
+    """Host-only: the work partition celes_setup would build; 'segments' is an int array [n][5] of
+    (cta, receiver block, e_begin, e_end, slot)."""
+    v = [ctypes.c_int() for _ in range(3)]
+    rc = lib().celes_plan_work(int(N), int(emitter_tile), int(resident_ctas), int(levels), int(emitter_splits),
+                               *[ctypes.byref(x) for x in v], None, 0)
+    if rc != CELES_OK:
+        raise CelesError(rc, "celes_plan_work")
+    seg = np.zeros((v[1].value, 5), dtype=np.int32)
+    rc = lib().celes_plan_work(int(N), int(emitter_tile), int(resident_ctas), int(levels), int(emitter_splits), None, None, None,
+                               seg.ctypes.data, seg.shape[0])
+    if rc != CELES_OK:
+        raise CelesError(rc, "celes_plan_work")
+    return {"ctas": v[0].value, "receivers_per_block": v[2].value, "segments": seg}
 
 
 def celes_translation_table(lmax: int):

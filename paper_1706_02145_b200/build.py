@@ -4,7 +4,7 @@
 
 ``--regen`` first re-runs both generators of the straight-line pair bodies, csrc/gen_coupling_body.py (direct sum,
 lmax 1-4) and csrc/gen_packed_body.py (packed rotated body, lmax 1-5); needs SymPy, the generated files are committed.
-nvcc cross-compiles without a GPU.  Four translation units (csrc/celes.cu, solve.cu, precond.cu, fields.cu).  The library is loaded by ``paper_1706_02145_b200.binding`` via ctypes.
+nvcc cross-compiles without a GPU.  Five translation units (csrc/celes.cu, solve.cu, precond.cu, fields.cu, probe.cu).  The library is loaded by ``paper_1706_02145_b200.binding`` via ctypes.
 """
 from __future__ import annotations
 
@@ -15,7 +15,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libceles.so")
-NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
+NVCC_FLAGS = ["-std=c++17", "-O3", *os.environ.get("CELES_NVCC_EXTRA", "").split(), "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-shared", "-Xcompiler", "-fPIC"]
 # cuSOLVER (LU of the preconditioner blocks); the CUDA toolkit's copy, found at run time through the rpath
 NVCC_LIBS = ["-lcusolver", "-Xlinker", "-rpath=/usr/local/cuda/lib64"]
@@ -41,8 +41,8 @@ def build(force: bool = False, regen: bool = False, verbose: bool = False) -> st
         subprocess.run([sys.executable, os.path.join(CSRC, "gen_packed_body.py")], check=True)
     if force or stale():
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-        units = [os.path.join(CSRC, f) for f in ("celes.cu", "solve.cu", "precond.cu", "fields.cu")]
-        cmd = [nvcc, *NVCC_FLAGS, "--threads", "4", *(["-Xptxas", "-v"] if verbose else []), "-o", LIB, *units, *NVCC_LIBS]
+        units = [os.path.join(CSRC, f) for f in ("celes.cu", "solve.cu", "precond.cu", "fields.cu", "probe.cu")]
+        cmd = [nvcc, *NVCC_FLAGS, "--threads", "5", *(["-Xptxas", "-v"] if verbose else []), "-o", LIB, *units, *NVCC_LIBS]
         subprocess.run(cmd, check=True)
     return LIB
 

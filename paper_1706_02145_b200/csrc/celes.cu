@@ -19,40 +19,52 @@
 #include "ctx.h"
 #include "coupling_kernel.cuh"
 #include "translation_table.h"
+#include "work_partition.h"
 
 namespace {
 
 using celes::kBlock;
 
-template <int LMAX, int ROT, bool TAB>
-int launch_coupling_tt(const celes_ctx* c, cudaStream_t s) {
+template <int LMAX, int ROT, bool TAB, bool EXT>
+int launch_coupling_tt(const celes_ctx* c, cudaStream_t s, int rb0, int rb1) {
     const size_t smem = celes::coupling_smem_bytes<LMAX>(c->etile);
-    dim3 grid(c->rblocks, c->splits);
-    celes::coupling_kernel<LMAX, ROT, TAB><<<grid, kBlock, smem, s>>>(c->N, c->chunk, c->etile, c->htab_desc, c->kpos,
-                                                                      c->bpm, c->ypart);
+    const int cta0 = c->h_cta_of_block_first[rb0], cta1 = c->h_cta_of_block_last[rb1];
+    celes::coupling_kernel<LMAX, ROT, TAB, EXT><<<cta1 - cta0 + 1, kBlock, smem, s>>>(
+        c->N, c->bs, c->etile, cta0, rb0, rb1, c->htab_desc, c->cta_begin, c->seg, c->kpos, c->bpm, c->ypart);
     return cudaGetLastError() == cudaSuccess ? CELES_OK : CELES_ECUDA;
 }
 
-template <int LMAX, int ROT, bool TAB>
+// The dynamic shared-memory limit is an attribute of the kernel for the whole process, not of a context: raise it once
+// to the device's opt-in maximum so that contexts with different emitter tiles never lower it for one another.
+template <int LMAX, int ROT, bool TAB, bool EXT>
 int prepare_coupling_tt(celes_ctx* c, int* ctas_per_sm) {
     const size_t smem = celes::coupling_smem_bytes<LMAX>(c->etile);
     c->coupling_smem = smem;
-    CU_TRY(cudaFuncSetAttribute(celes::coupling_kernel<LMAX, ROT, TAB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, celes::coupling_kernel<LMAX, ROT, TAB>, kBlock, smem));
+    int optin = 0;
+    CU_TRY(cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, c->device));
+    if (smem > (size_t)optin) return CELES_EINVAL;             // emitter tile too large for this lmax
+    CU_TRY(cudaFuncSetAttribute(celes::coupling_kernel<LMAX, ROT, TAB, EXT>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin));
+    CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, celes::coupling_kernel<LMAX, ROT, TAB, EXT>, kBlock, smem));
     return CELES_OK;
 }
 
-// the table look-up exists for the default (packed rotated) body only
+// the table look-up and the extended range mode exist for the default (packed rotated) body only
 template <int LMAX, int ROT>
-int launch_coupling_t(const celes_ctx* c, cudaStream_t s) {
-    if constexpr (ROT == celes::kRotated) { if (c->htab) return launch_coupling_tt<LMAX, ROT, true>(c, s); }
-    return launch_coupling_tt<LMAX, ROT, false>(c, s);
+int launch_coupling_t(const celes_ctx* c, cudaStream_t s, int rb0, int rb1) {
+    if constexpr (ROT == celes::kRotated) {
+        if (c->htab) return launch_coupling_tt<LMAX, ROT, true, false>(c, s, rb0, rb1);
+        if (c->extended_range) return launch_coupling_tt<LMAX, ROT, false, true>(c, s, rb0, rb1);
+    }
+    return launch_coupling_tt<LMAX, ROT, false, false>(c, s, rb0, rb1);
 }
 
 template <int LMAX, int ROT>
 int prepare_coupling_t(celes_ctx* c, int* ctas_per_sm) {
-    if constexpr (ROT == celes::kRotated) { if (c->htab) return prepare_coupling_tt<LMAX, ROT, true>(c, ctas_per_sm); }
-    return prepare_coupling_tt<LMAX, ROT, false>(c, ctas_per_sm);
+    if constexpr (ROT == celes::kRotated) {
+        if (c->htab) return prepare_coupling_tt<LMAX, ROT, true, false>(c, ctas_per_sm);
+        if (c->extended_range) return prepare_coupling_tt<LMAX, ROT, false, true>(c, ctas_per_sm);
+    }
+    return prepare_coupling_tt<LMAX, ROT, false, false>(c, ctas_per_sm);
 }
 
 #define CELES_DISPATCH(fn, ...)                                                            \
@@ -65,25 +77,30 @@ int prepare_coupling_t(celes_ctx* c, int* ctas_per_sm) {
     }                                                                                      \
     return CELES_EINVAL
 
-int launch_coupling(const celes_ctx* c, cudaStream_t s) { CELES_DISPATCH(launch_coupling_t, c, s); }
+int launch_coupling(const celes_ctx* c, cudaStream_t s, int rb0, int rb1) { CELES_DISPATCH(launch_coupling_t, c, s, rb0, rb1); }
 int prepare_coupling(celes_ctx* c, int* ctas_per_sm) { CELES_DISPATCH(prepare_coupling_t, c, ctas_per_sm); }
 
 // y = W b (tdiag == nullptr) or out = b - T (W b): pack -> coupling -> finalize, all on stream s.
 }  // namespace
 
-int celes::host::run_matvec(celes_ctx* c, const float2* b, float2* out, bool system, cudaStream_t s) {
+int celes::host::run_matvec(celes_ctx* c, const float2* b, float2* out, bool system, cudaStream_t s, int row_begin,
+                            int row_end) {
+    if (row_begin < 0 || row_end > c->N || row_begin >= row_end) return CELES_EINVAL;
     const int H = c->nmax / 2;
     const long long nh = (long long)c->N * H;
     const int tb = 256;
-    const unsigned gb = (unsigned)((nh + tb - 1) / tb);
+    const unsigned gb = (unsigned)((nh + tb - 1) / tb);                      // every emitter's b is needed
+    const unsigned gf = (unsigned)(((long long)(row_end - row_begin) * H + tb - 1) / tb);
     if (c->variant == celes::kRotated) celes::pack_kernel<celes::kRotated><<<gb, tb, 0, s>>>(c->N, H, b, c->bpm);
     else celes::pack_kernel<celes::kDirect><<<gb, tb, 0, s>>>(c->N, H, b, c->bpm);
     if (cudaGetLastError() != cudaSuccess) return CELES_ECUDA;
-    int rc = launch_coupling(c, s);
+    int rc = launch_coupling(c, s, row_begin / c->bs, (row_end - 1) / c->bs);
     if (rc) return rc;
     const float2* td = system ? c->tdiag : nullptr;
-    if (c->variant == celes::kRotated) celes::finalize_kernel<celes::kRotated><<<gb, tb, 0, s>>>(c->N, H, c->splits, c->ypart, td, b, out);
-    else celes::finalize_kernel<celes::kDirect><<<gb, tb, 0, s>>>(c->N, H, c->splits, c->ypart, td, b, out);
+    if (c->variant == celes::kRotated)
+        celes::finalize_kernel<celes::kRotated><<<gf, tb, 0, s>>>(row_begin, row_end, H, c->bs, c->slot_begin, c->ypart, td, b, out);
+    else
+        celes::finalize_kernel<celes::kDirect><<<gf, tb, 0, s>>>(row_begin, row_end, H, c->bs, c->slot_begin, c->ypart, td, b, out);
     return cudaGetLastError() == cudaSuccess ? CELES_OK : CELES_ECUDA;
 }
 
@@ -137,85 +154,9 @@ void free_ctx(celes_ctx* c) {
     if (!c) return;
     celes::host::free_precond(c);
     celes::host::free_krylov(c);
-    cudaFree(c->kpos); cudaFree(c->tdiag); cudaFree(c->bpm); cudaFree(c->ypart); cudaFree(c->htab); cudaFree(c->host_in); cudaFree(c->host_out);
+    cudaFree(c->cta_begin); cudaFree(c->seg); cudaFree(c->slot_begin);
+    cudaFree(c->kpos); cudaFree(c->tdiag); cudaFree(c->bpm); cudaFree(c->ypart); cudaFree(c->htab); cudaFree(c->host_in); cudaFree(c->host_out); cudaFree(c->scratch);
     delete c;
-}
-
-// ---- FP32 peak probe kernels -----------------------------------------------------------------------------
-template <int VARIANT>
-__global__ void __launch_bounds__(256) ffma_probe_kernel(int iters, float seed, float* sink) {
-    constexpr int C = 16;                         // independent chains per thread
-    float a[C];
-#pragma unroll
-    for (int c = 0; c < C; ++c) a[c] = seed + (float)(threadIdx.x + c);
-    const float m = 0.999f + seed * 1e-9f, d = seed * 1e-3f;
-    for (int it = 0; it < iters; ++it) {
-#pragma unroll
-        for (int u = 0; u < 8; ++u) {
-            if (VARIANT == 0) {
-#pragma unroll
-                for (int c = 0; c < C; ++c) a[c] = fmaf(a[c], m, d);
-            } else if (VARIANT == 1) {
-#pragma unroll
-                for (int c = 0; c < C; ++c) a[c] = fmaf(a[c], 0.99951171875f, d);
-            } else {
-#pragma unroll
-                for (int c = 0; c < C; c += 2) {
-                    unsigned long long acc, mm, dd;
-                    asm("mov.b64 %0, {%1, %2};" : "=l"(acc) : "f"(a[c]), "f"(a[c + 1]));
-                    asm("mov.b64 %0, {%1, %1};" : "=l"(mm) : "f"(m));
-                    asm("mov.b64 %0, {%1, %1};" : "=l"(dd) : "f"(d));
-                    asm("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(acc) : "l"(mm), "l"(dd));
-                    asm("mov.b64 {%0, %1}, %2;" : "=f"(a[c]), "=f"(a[c + 1]) : "l"(acc));
-                }
-            }
-        }
-    }
-    float t = 0.f;
-#pragma unroll
-    for (int c = 0; c < C; ++c) t += a[c];
-    if (t == 12345.678f) sink[0] = t;             // never true in practice; keeps the chains alive
-}
-
-// Variants 3 / 4: packed fma.rn.f32x2 streams shaped like the pair body (a real coefficient times a packed complex
-// value added to a packed accumulator, eight independent accumulators), in a fixed instruction order (asm
-// volatile).  3: consecutive instructions share no source register (every operand is fetched from the register
-// file); 4: eight consecutive instructions share the packed value (operand reuse cache).  They measure what the
-// FMA pipe sustains when three register operands per instruction have to be delivered.
-template <int SHARE>
-__global__ void __launch_bounds__(128) ffma2_operand_probe_kernel(int iters, const float2* __restrict__ in, float* sink) {
-    typedef unsigned long long u64;
-    u64 R[8], z[4], u[8];
-#pragma unroll
-    for (int c = 0; c < 8; ++c) {
-        const float r = in[(threadIdx.x + c) & 63].x;
-        asm("mov.b64 %0, {%1, %1};" : "=l"(R[c]) : "f"(r));
-        asm("mov.b64 %0, {%1, %1};" : "=l"(u[c]) : "f"(0.0f));
-    }
-#pragma unroll
-    for (int c = 0; c < 4; ++c) {
-        const float2 v = in[(threadIdx.x + 8 + c) & 63];
-        asm("mov.b64 %0, {%1, %2};" : "=l"(z[c]) : "f"(v.x), "f"(v.y));
-    }
-    for (int it = 0; it < iters; ++it) {
-#pragma unroll
-        for (int rep = 0; rep < 4; ++rep)
-#pragma unroll
-            for (int m = 0; m < 4; ++m)
-#pragma unroll
-                for (int t = 0; t < 8; ++t) {
-                    if (SHARE) asm volatile("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(u[t]) : "l"(R[(t + m) & 7]), "l"(z[m]));
-                    else asm volatile("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(u[t]) : "l"(R[(t + m) & 7]), "l"(z[(t + m) & 3]));
-                }
-    }
-    float acc = 0.f;
-#pragma unroll
-    for (int c = 0; c < 8; ++c) {
-        float a, b;
-        asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(u[c]));
-        acc += a + b;
-    }
-    if (acc == 12345.678f) sink[0] = acc;
 }
 
 }  // namespace
@@ -239,7 +180,7 @@ const char* celes_strerror(int code) {
     return "unknown error code";
 }
 
-int celes_translation_table(int lmax, double* a5_re, double* b5_im) {
+static int translation_table_impl(int lmax, double* a5_re, double* b5_im) {
     if (lmax < CELES_LMAX_MIN || lmax > CELES_LMAX_MAX || !a5_re || !b5_im) return CELES_EINVAL;
     std::vector<double> a, b;
     if (!celes::build_translation_table(lmax, a, b)) return CELES_EINVAL;
@@ -248,8 +189,16 @@ int celes_translation_table(int lmax, double* a5_re, double* b5_im) {
     return CELES_OK;
 }
 
-int celes_setup(celes_ctx** out, int N, int lmax, const double* pos_xyz, const double* radii, const double* mie_q,
-                double k, const celes_options* opt, void* cuda_stream) {
+int celes_translation_table(int lmax, double* a5_re, double* b5_im) { CELES_NOTHROW(translation_table_impl(lmax, a5_re, b5_im)) }
+
+// the context under construction: released on every exit but the successful one (exceptions included)
+struct CtxHolder {
+    celes_ctx* c = nullptr;
+    ~CtxHolder() { free_ctx(c); }
+};
+
+static int setup_impl(celes_ctx** out, int N, int lmax, const double* pos_xyz, const double* radii, const double* mie_q,
+                      double k, const celes_options* opt, void* cuda_stream) {
     if (!out) return CELES_EINVAL;
     *out = nullptr;
     if (N < 1 || lmax < CELES_LMAX_MIN || lmax > CELES_LMAX_MAX || !pos_xyz || !radii || !mie_q) return CELES_EINVAL;
@@ -261,29 +210,40 @@ int celes_setup(celes_ctx** out, int N, int lmax, const double* pos_xyz, const d
     for (long long t = 0; t < 4LL * N * lmax; ++t) if (!std::isfinite(mie_q[t])) return CELES_EINVAL;
     const bool skip = opt && opt->skip_overlap_check;
     if (!skip && !spheres_disjoint(N, pos_xyz, radii)) return CELES_EINVAL;
-    if (opt && (opt->emitter_tile < 0 || opt->emitter_splits < 0 || opt->emitter_tile > 128)) return CELES_EINVAL;
+    if (opt && (opt->emitter_tile < 0 || opt->emitter_splits < 0 || opt->emitter_tile > 128 || opt->levels < 0)) return CELES_EINVAL;
     if (opt && (opt->translation < 0 || opt->translation > CELES_TRANSLATION_DIRECT)) return CELES_EINVAL;
     if (lmax > 4 && opt && opt->translation != CELES_TRANSLATION_ROTATED) return CELES_EINVAL;   // one body at lmax = 5
     const bool table = opt && opt->hankel == CELES_HANKEL_TABLE;
+    if (opt && (opt->range < CELES_RANGE_AUTO || opt->range > CELES_RANGE_EXTENDED)) return CELES_EINVAL;
+    if (opt && opt->range == CELES_RANGE_EXTENDED && (table || opt->translation != CELES_TRANSLATION_ROTATED)) return CELES_EINVAL;
     if (opt && opt->hankel != CELES_HANKEL_REGISTERS && opt->hankel != CELES_HANKEL_TABLE) return CELES_EINVAL;
     if (table && (opt->translation != CELES_TRANSLATION_ROTATED || !(opt->hankel_dr >= 0.0) || !std::isfinite(opt->hankel_dr)))
         return CELES_EINVAL;
 
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); return CELES_ECUDA; }
-    celes_ctx* c = new (std::nothrow) celes_ctx;
+    CtxHolder holder;
+    celes_ctx* c = holder.c = new (std::nothrow) celes_ctx;
     if (!c) return CELES_ENOMEM;
     cudaStream_t s = (cudaStream_t)cuda_stream;
     c->N = N; c->lmax = lmax; c->nmax = nmax; c->k = k;
     int rc = CELES_OK;
-    auto fail = [&](int code) { free_ctx(c); return code; };
+    auto fail = [&](int code) { return code; };                 // the holder releases the context
     if (cudaGetDevice(&c->device) != cudaSuccess) return fail(CELES_ECUDA);
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, c->device) != cudaSuccess) return fail(CELES_ECUDA);
     c->sm_count = prop.multiProcessorCount;
     c->etile = (opt && opt->emitter_tile > 0) ? opt->emitter_tile : 32;
     c->variant = opt ? opt->translation : CELES_TRANSLATION_ROTATED;
-    c->rblocks = (N + kBlock - 1) / kBlock;
+    {   // extent of the cluster in units of 1/k: decides the range mode (celes.h: celes_options.range)
+        double lo[3] = {pos_xyz[0], pos_xyz[1], pos_xyz[2]}, hi[3] = {pos_xyz[0], pos_xyz[1], pos_xyz[2]};
+        for (int i = 0; i < N; ++i)
+            for (int a = 0; a < 3; ++a) { lo[a] = std::min(lo[a], pos_xyz[3 * i + a]); hi[a] = std::max(hi[a], pos_xyz[3 * i + a]); }
+        c->kd_max = k * std::sqrt((hi[0] - lo[0]) * (hi[0] - lo[0]) + (hi[1] - lo[1]) * (hi[1] - lo[1]) + (hi[2] - lo[2]) * (hi[2] - lo[2]));
+        const int range = opt ? opt->range : CELES_RANGE_AUTO;
+        const bool can = !table && c->variant == celes::kRotated;
+        c->extended_range = can && (range == CELES_RANGE_EXTENDED || (range == CELES_RANGE_AUTO && c->kd_max > CELES_RANGE_AUTO_KD));
+    }
     if (table) {
         // S2: h_p^(1)(k r) for r from the smallest possible centre distance (two touching spheres of
         // the smallest radius; spheres are disjoint) to the diagonal of the centres' bounding box, spacing dr; FP64
@@ -325,27 +285,18 @@ int celes_setup(celes_ctx** out, int N, int lmax, const double* pos_xyz, const d
     rc = prepare_coupling(c, &ctas_per_sm);
     if (rc) return fail(rc);
     ctas_per_sm = std::max(1, ctas_per_sm);
-    if (opt && opt->emitter_splits > 0) {
-        c->splits = std::min(opt->emitter_splits, N);
-    } else {
-        // Split the emitter sum so that the grid is a whole number of waves (slots = SMs x resident CTAs): among
-        // 1..16 waves take the split with the best fill (all CTAs do equal work, so a full last wave means no
-        // tail), slightly preferring more waves, with at least 96 emitters per CTA.
-        const long long slots = (long long)c->sm_count * ctas_per_sm;
-        const long long maxsp = std::max<long long>(1, N / 96);
-        long long best = 1;
-        double best_score = -1.0;
-        for (long long waves = 1; waves <= 16; ++waves) {
-            const long long sp = std::min(maxsp, std::max<long long>(1, (waves * slots) / c->rblocks));
-            const long long used_waves = (sp * c->rblocks + slots - 1) / slots;
-            const double eff = (double)sp * c->rblocks / ((double)used_waves * slots);
-            const double score = eff - 0.02 / (double)used_waves;
-            if (score > best_score + 1e-12) { best_score = score; best = sp; }
-        }
-        c->splits = (int)best;
-    }
-    c->chunk = (N + c->splits - 1) / c->splits;
-    c->splits = (N + c->chunk - 1) / c->chunk;
+    // work partition (work_partition.h): guided runs over the flattened (receiver block, emitter tile) grid, or the
+    // caller's fixed number of emitter splits per receiver block
+    c->fixed_splits = (opt && opt->emitter_splits > 0) ? opt->emitter_splits : 0;
+    const int levels = (opt && opt->levels > 0) ? std::min(opt->levels, 16) : CELES_DEFAULT_LEVELS;
+    celes::WorkPartition wp = celes::build_partition(N, kBlock, c->etile, c->sm_count * ctas_per_sm, levels, c->fixed_splits);
+    c->bs = wp.bs; c->rblocks = wp.rblocks; c->n_cta = wp.n_cta; c->n_seg = (int)wp.seg.size();
+    c->h_cta_of_block_first.assign(wp.rblocks, 0);
+    c->h_cta_of_block_last.assign(wp.rblocks, 0);
+    for (int cta = wp.n_cta - 1; cta >= 0; --cta)
+        for (int t = wp.cta_begin[cta]; t < wp.cta_begin[cta + 1]; ++t) c->h_cta_of_block_first[wp.seg[t].rblock] = cta;
+    for (int cta = 0; cta < wp.n_cta; ++cta)
+        for (int t = wp.cta_begin[cta]; t < wp.cta_begin[cta + 1]; ++t) c->h_cta_of_block_last[wp.seg[t].rblock] = cta;
 
     const size_t n = (size_t)N * nmax;
     c->pos.assign(pos_xyz, pos_xyz + 3 * (size_t)N);
@@ -368,13 +319,26 @@ int celes_setup(celes_ctx** out, int N, int lmax, const double* pos_xyz, const d
     SETUP_TRY(cudaMalloc(&c->kpos, sizeof(double) * kp.size()));
     SETUP_TRY(cudaMalloc(&c->tdiag, sizeof(float2) * n));
     SETUP_TRY(cudaMalloc(&c->bpm, sizeof(float2) * n));
-    SETUP_TRY(cudaMalloc(&c->ypart, sizeof(float2) * n * c->splits));
+    SETUP_TRY(cudaMalloc(&c->ypart, sizeof(float2) * (size_t)c->n_seg * kBlock * nmax));
+    SETUP_TRY(cudaMalloc(&c->cta_begin, sizeof(int) * wp.cta_begin.size()));
+    SETUP_TRY(cudaMalloc(&c->seg, sizeof(int4) * wp.seg.size()));
+    SETUP_TRY(cudaMalloc(&c->slot_begin, sizeof(int) * wp.slot_begin.size()));
+    static_assert(sizeof(celes::Segment) == sizeof(int4), "Segment is read as int4 on the device");
+    SETUP_TRY(cudaMemcpyAsync(c->cta_begin, wp.cta_begin.data(), sizeof(int) * wp.cta_begin.size(), cudaMemcpyHostToDevice, s));
+    SETUP_TRY(cudaMemcpyAsync(c->seg, wp.seg.data(), sizeof(int4) * wp.seg.size(), cudaMemcpyHostToDevice, s));
+    SETUP_TRY(cudaMemcpyAsync(c->slot_begin, wp.slot_begin.data(), sizeof(int) * wp.slot_begin.size(), cudaMemcpyHostToDevice, s));
     SETUP_TRY(cudaMemcpyAsync(c->kpos, kp.data(), sizeof(double) * kp.size(), cudaMemcpyHostToDevice, s));
     SETUP_TRY(cudaMemcpyAsync(c->tdiag, td.data(), sizeof(float2) * n, cudaMemcpyHostToDevice, s));
     SETUP_TRY(cudaStreamSynchronize(s));
 #undef SETUP_TRY
     *out = c;
+    holder.c = nullptr;
     return CELES_OK;
+}
+
+int celes_setup(celes_ctx** out, int N, int lmax, const double* pos_xyz, const double* radii, const double* mie_q,
+                double k, const celes_options* opt, void* cuda_stream) {
+    CELES_NOTHROW(setup_impl(out, N, lmax, pos_xyz, radii, mie_q, k, opt, cuda_stream))
 }
 
 int celes_coupling_matvec(celes_ctx* ctx, const void* b_dev, void* y_dev, void* cuda_stream) {
@@ -415,54 +379,67 @@ int celes_launch_config(const celes_ctx* ctx, int* receiver_blocks, int* emitter
                         int* emitter_tile) {
     if (!ctx) return CELES_EINVAL;
     if (receiver_blocks) *receiver_blocks = ctx->rblocks;
-    if (emitter_splits) *emitter_splits = ctx->splits;
+    if (emitter_splits) *emitter_splits = ctx->fixed_splits;
     if (block_threads) *block_threads = kBlock;
     if (emitter_tile) *emitter_tile = ctx->etile;
     return CELES_OK;
 }
 
-void celes_destroy(celes_ctx* ctx) { free_ctx(ctx); }
-
-int celes_fp32_peak_probe(int variant, int iters, double* flops_per_s, double* milliseconds, void* cuda_stream) {
-    if (variant < 0 || variant > 4 || iters < 1) return CELES_EINVAL;
-    int ndev = 0;
-    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); return CELES_ECUDA; }
-    cudaStream_t s = (cudaStream_t)cuda_stream;
-    int dev = 0;
-    cudaDeviceProp prop;
-    CU_TRY(cudaGetDevice(&dev));
-    CU_TRY(cudaGetDeviceProperties(&prop, dev));
-    float* sink = nullptr;
-    CU_TRY(cudaMalloc(&sink, sizeof(float)));
-    float2* zeros = nullptr;
-    if (cudaMalloc(&zeros, 64 * sizeof(float2)) != cudaSuccess) { cudaFree(sink); return CELES_ENOMEM; }
-    cudaMemsetAsync(zeros, 0, 64 * sizeof(float2), s);
-    const bool operand = variant >= 3;
-    const int blocks = prop.multiProcessorCount * (operand ? 4 : 8), threads = operand ? 128 : 256;
-    cudaEvent_t e0, e1;
-    cudaEventCreate(&e0); cudaEventCreate(&e1);
-    auto launch = [&](int it) {
-        if (variant == 0) ffma_probe_kernel<0><<<blocks, threads, 0, s>>>(it, 1.0f, sink);
-        else if (variant == 1) ffma_probe_kernel<1><<<blocks, threads, 0, s>>>(it, 1.0f, sink);
-        else if (variant == 2) ffma_probe_kernel<2><<<blocks, threads, 0, s>>>(it, 1.0f, sink);
-        else if (variant == 3) ffma2_operand_probe_kernel<0><<<blocks, threads, 0, s>>>(it, zeros, sink);
-        else ffma2_operand_probe_kernel<1><<<blocks, threads, 0, s>>>(it, zeros, sink);
-    };
-    launch(std::max(1, iters / 10));              // warm-up
-    cudaEventRecord(e0, s);
-    launch(iters);
-    cudaEventRecord(e1, s);
-    int rc = CELES_OK;
-    if (cudaEventSynchronize(e1) != cudaSuccess || cudaGetLastError() != cudaSuccess) rc = CELES_ECUDA;
-    float ms = 0.f;
-    cudaEventElapsedTime(&ms, e0, e1);
-    cudaEventDestroy(e0); cudaEventDestroy(e1);
-    cudaFree(sink);
-    cudaFree(zeros);
-    const double fmas = (double)blocks * threads * (operand ? 256.0 : 128.0) * (double)iters;   // FMAs per thread and iteration
-    if (flops_per_s) *flops_per_s = 2.0 * fmas / (ms * 1e-3);
-    if (milliseconds) *milliseconds = ms;
-    return rc;
+#ifdef CELES_TRACE
+int celes_debug_trace(unsigned long long* out) {
+    return cudaMemcpyFromSymbol(out, celes::g_trace, sizeof(unsigned long long) * 3 * 8192) == cudaSuccess ? CELES_OK : CELES_ECUDA;
 }
+#endif
+
+int celes_range_info(const celes_ctx* ctx, double* kd_max, int* extended) {
+    if (!ctx) return CELES_EINVAL;
+    if (kd_max) *kd_max = ctx->kd_max;
+    if (extended) *extended = ctx->extended_range ? 1 : 0;
+    return CELES_OK;
+}
+
+int celes_work_partition(const celes_ctx* ctx, int* ctas, int* segments, int* receivers_per_block) {
+    if (!ctx) return CELES_EINVAL;
+    if (ctas) *ctas = ctx->n_cta;
+    if (segments) *segments = ctx->n_seg;
+    if (receivers_per_block) *receivers_per_block = ctx->bs;
+    return CELES_OK;
+}
+
+int celes_plan_work(int N, int emitter_tile, int resident_ctas, int levels, int emitter_splits, int* ctas, int* segments,
+                    int* receivers_per_block, int* seg_out, int seg_capacity) {
+    if (N < 1 || emitter_tile < 1 || resident_ctas < 1 || emitter_splits < 0 || levels < 0) return CELES_EINVAL;
+    try {
+        const celes::WorkPartition wp = celes::build_partition(N, kBlock, emitter_tile, resident_ctas,
+                                                               levels > 0 ? levels : CELES_DEFAULT_LEVELS, emitter_splits);
+        if (ctas) *ctas = wp.n_cta;
+        if (segments) *segments = (int)wp.seg.size();
+        if (receivers_per_block) *receivers_per_block = wp.bs;
+        if (seg_out) {
+            if (seg_capacity < (int)wp.seg.size()) return CELES_EINVAL;
+            for (int cta = 0; cta < wp.n_cta; ++cta)
+                for (int t = wp.cta_begin[cta]; t < wp.cta_begin[cta + 1]; ++t) {
+                    const celes::Segment& sg = wp.seg[t];
+                    int* o = seg_out + 5 * (size_t)t;
+                    o[0] = cta; o[1] = sg.rblock; o[2] = sg.e_begin; o[3] = sg.e_end; o[4] = sg.slot;
+                }
+        }
+    } catch (const std::bad_alloc&) {
+        return CELES_ENOMEM;
+    }
+    return CELES_OK;
+}
+
+int celes_coupling_matvec_rows(celes_ctx* ctx, int row_begin, int row_end, const void* b_dev, void* y_rows_dev, void* cuda_stream) {
+    if (!ctx || !b_dev || !y_rows_dev || b_dev == y_rows_dev) return CELES_EINVAL;
+    return run_matvec(ctx, (const float2*)b_dev, (float2*)y_rows_dev, false, (cudaStream_t)cuda_stream, row_begin, row_end);
+}
+
+int celes_system_matvec_rows(celes_ctx* ctx, int row_begin, int row_end, const void* b_dev, void* out_rows_dev, void* cuda_stream) {
+    if (!ctx || !b_dev || !out_rows_dev || b_dev == out_rows_dev) return CELES_EINVAL;
+    return run_matvec(ctx, (const float2*)b_dev, (float2*)out_rows_dev, true, (cudaStream_t)cuda_stream, row_begin, row_end);
+}
+
+void celes_destroy(celes_ctx* ctx) { free_ctx(ctx); }
 
 }  // extern "C"

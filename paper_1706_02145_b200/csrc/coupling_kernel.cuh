@@ -5,8 +5,9 @@
 //                                                  (packed variant: w_m = i u-_m in place of u-_m)
 //   coupling_kernel  tiled (receiver-block x emitter-block) translation; one thread per receiver, the
 //                    emitter tile (coefficients + FP64 centres) staged through shared memory, FP32 complex
-//                    accumulation in registers (lmax <= 3) or in a conflict-free shared-memory slab (lmax = 4)
-//   finalize_kernel  sums the emitter splits, undoes the +- transform, optional epilogue out = b - T y (eq. 9)
+//                    accumulation in registers (lmax <= 3) or in a conflict-free shared-memory slab (lmax >= 4);
+//                    which (receiver block, emitter range) pieces a CTA does comes from work_partition.h
+//   finalize_kernel  sums the partial-sum slots, undoes the basis transform, optional epilogue out = b - T y (eq. 9)
 #pragma once
 #include <cuda_runtime.h>
 
@@ -23,6 +24,9 @@ namespace celes {
 #define CELES_COUPLING_BOUNDS __launch_bounds__(CELES_KBLOCK)
 #endif
 constexpr int kBlock = CELES_KBLOCK;   // receivers (threads) per CTA
+#ifdef CELES_TRACE
+__device__ unsigned long long g_trace[3 * 8192];   // diagnostic builds: (smid, start ns, end ns) per CTA
+#endif
 
 __host__ __device__ constexpr int nmax_of(int lmax) { return 2 * lmax * (lmax + 2); }
 
@@ -116,17 +120,32 @@ struct YPolicy<4> { using type = YSmem<nmax_of(4)>; };
 template <>
 struct YPolicy<5> { using type = YSmem<nmax_of(5)>; };
 
+// accumulator slab (lmax >= 4) + two emitter tiles (double buffer): coefficients [etile][nmax] and centres [etile][3]
 template <int LMAX>
 constexpr size_t coupling_smem_bytes(int etile) {
-    return YPolicy<LMAX>::type::smem_bytes() + (size_t)etile * (nmax_of(LMAX) * sizeof(float2) + 3 * sizeof(double));
+    return YPolicy<LMAX>::type::smem_bytes() + 2 * (size_t)etile * (nmax_of(LMAX) * sizeof(float2) + 3 * sizeof(double));
 }
 
+// Asynchronous global -> shared copies (cp.async, SASS LDGSTS): the next emitter tile is fetched while the current one
+// is being translated, with no register staging and every request of the tile in flight at once.
+__device__ __forceinline__ void cp_async_16(void* smem, const void* gmem) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(smem)), "l"(gmem));
+}
+__device__ __forceinline__ void cp_async_8(void* smem, const void* gmem) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((unsigned)__cvta_generic_to_shared(smem)), "l"(gmem));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
 // ---------------------------------------------------------------------------------------------------------
-// grid = (ceil(N / kBlock), splits).  CTA (bx, by) translates emitters [by*chunk, min(N, (by+1)*chunk)) to
-// receivers bx*kBlock + tid and writes its partial sums to ypart[by][receiver][q].
+// grid = CTAs of the work partition (work_partition.h), cta0 + blockIdx.x is the CTA's entry in the table.  A CTA walks
+// its segments: segment (rblock, [e_begin, e_end), slot) translates those emitters to receivers rblock*bs + tid,
+// tid < bs, from fresh accumulators, and writes them to ypart[slot][tid][q].  Segments of receiver blocks outside
+// [rb0, rb1] are skipped (row-slice calls).
 //   kpos  [N][3] FP64: k * r_i.  The subtraction r_i - r_i' is done in FP64, everything after it in FP32.
-template <int LMAX, int VARIANT, bool TABLE>
-__global__ void CELES_COUPLING_BOUNDS coupling_kernel(int N, int chunk, int etile, HankelTable htab,
+template <int LMAX, int VARIANT, bool TABLE, bool EXT>
+__global__ void CELES_COUPLING_BOUNDS coupling_kernel(int N, int bs, int etile, int cta0, int rb0, int rb1, HankelTable htab,
+                                                          const int* __restrict__ cta_begin, const int4* __restrict__ seg,
                                                           const double* __restrict__ kpos,
                                                           const float2* __restrict__ bpm,
                                                           float2* __restrict__ ypart) {
@@ -134,68 +153,102 @@ __global__ void CELES_COUPLING_BOUNDS coupling_kernel(int N, int chunk, int etil
     using Y = typename YPolicy<LMAX>::type;
     extern __shared__ __align__(16) float smem_raw[];
     float* ysm = smem_raw;
-    float2* sb = reinterpret_cast<float2*>(reinterpret_cast<char*>(smem_raw) + Y::smem_bytes());   // [etile][NMAX]
-    double* spos = reinterpret_cast<double*>(sb + (size_t)etile * NMAX);                           // [etile][3]
+    float2* sb = reinterpret_cast<float2*>(reinterpret_cast<char*>(smem_raw) + Y::smem_bytes());   // [2][etile][NMAX]
+    double* spos = reinterpret_cast<double*>(sb + 2 * (size_t)etile * NMAX);                       // [2][etile][3]
+    // H1: stage emitters [t0, t0 + ne) into buffer `buf` -- the coefficients are contiguous in global memory
+    // (ne * NMAX float2 = ne * NMAX / 2 sixteen-byte pieces), the FP64 centres in eight-byte pieces
+    auto stage = [&](int t0, int ne, int buf) {
+        const float4* src = reinterpret_cast<const float4*>(bpm + (size_t)t0 * NMAX);
+        float4* dst = reinterpret_cast<float4*>(sb + (size_t)buf * etile * NMAX);
+        const int nvec = ne * NMAX / 2;
+        for (int v = threadIdx.x; v < nvec; v += kBlock) cp_async_16(dst + v, src + v);
+        double* dpos = spos + (size_t)buf * etile * 3;
+        for (int v = threadIdx.x; v < 3 * ne; v += kBlock) cp_async_8(dpos + v, kpos + (size_t)3 * t0 + v);
+        cp_async_commit();
+    };
 
     const int tid = threadIdx.x;
-    const int i = blockIdx.x * kBlock + tid;
-    const bool active = i < N;
-    const int ic = active ? i : N - 1;
-    const double xi = kpos[3 * ic], yi = kpos[3 * ic + 1], zi = kpos[3 * ic + 2];
+    const int cta = cta0 + blockIdx.x;
+#ifdef CELES_TRACE
+    unsigned long long trace_t0 = 0;
+    if (tid == 0) asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(trace_t0));
+#endif
+    const int s_end = cta_begin[cta + 1];
+    for (int sidx = cta_begin[cta]; sidx < s_end; ++sidx) {
+        const int4 sg = seg[sidx];                             // (rblock, e_begin, e_end, slot)
+        if (sg.x < rb0 || sg.x > rb1) continue;
+        const int i = sg.x * bs + tid;
+        const bool active = tid < bs && i < N;
+        const int ic = active ? i : N - 1;
+        const double xi = kpos[3 * ic], yi = kpos[3 * ic + 1], zi = kpos[3 * ic + 2];
 
-    Y yacc;
-    yacc.init(ysm, tid);
+        Y yacc;
+        yacc.init(ysm, tid);
 
-    const int e_begin = blockIdx.y * chunk;
-    const int e_end = min(N, e_begin + chunk);
-    for (int t0 = e_begin; t0 < e_end; t0 += etile) {
-        const int ne = min(etile, e_end - t0);
-        __syncthreads();                                       // previous tile fully consumed
-        {   // H1: stage the tile -- coefficients are contiguous in global memory: ne * NMAX float2 = ne*NMAX/2 float4
-            const float4* src = reinterpret_cast<const float4*>(bpm + (size_t)t0 * NMAX);
-            float4* dst = reinterpret_cast<float4*>(sb);
-            const int nvec = ne * NMAX / 2;
-            for (int v = tid; v < nvec; v += kBlock) dst[v] = __ldg(src + v);
-            for (int v = tid; v < 3 * ne; v += kBlock) spos[v] = kpos[(size_t)3 * t0 + v];
+        __syncthreads();                                           // the previous segment's last tile is consumed
+        stage(sg.y, min(etile, sg.z - sg.y), 0);
+        int buf = 0;
+        for (int t0 = sg.y; t0 < sg.z; t0 += etile, buf ^= 1) {
+            const int ne = min(etile, sg.z - t0);
+            cp_async_wait_all();
+            __syncthreads();                                       // tile t0 has landed; tile t0 - etile is consumed
+            if (t0 + etile < sg.z) stage(t0 + etile, min(etile, sg.z - t0 - etile), buf ^ 1);
+            const float2* tb = sb + (size_t)buf * etile * NMAX;
+            const double* tp = spos + (size_t)buf * etile * 3;
+            for (int e = 0; e < ne; ++e) {
+                if (t0 + e == i) continue;                         // sum over i' != i (eq. 6)
+                const double dx = xi - tp[3 * e];                  // d = r_i - r_i' (eq. 7), FP64 subtraction
+                const double dy = yi - tp[3 * e + 1];
+                const double dz = zi - tp[3 * e + 2];
+                const float2* be = tb + e * NMAX;
+                auto bload = [be](int q) { return be[q]; };        // same address in every lane: LDS broadcast
+                pair_translate<LMAX, VARIANT, TABLE, EXT>(dx, dy, dz, htab, bload, yacc);
+            }
         }
-        __syncthreads();
-        for (int e = 0; e < ne; ++e) {
-            if (t0 + e == i) continue;                         // sum over i' != i (eq. 6)
-            const float dx = (float)(xi - spos[3 * e]);        // d = r_i - r_i' (eq. 7), FP64 subtraction
-            const float dy = (float)(yi - spos[3 * e + 1]);
-            const float dz = (float)(zi - spos[3 * e + 2]);
-            const float2* be = sb + e * NMAX;
-            auto bload = [be](int q) { return be[q]; };        // same address in every lane: LDS broadcast
-            pair_translate<LMAX, VARIANT, TABLE>(dx, dy, dz, htab, bload, yacc);
-        }
-    }
-    if (active) {
-        float2* dst = ypart + ((size_t)blockIdx.y * N + i) * NMAX;
+        if (active) {
+            float4* dst = reinterpret_cast<float4*>(ypart + ((size_t)sg.w * kBlock + tid) * NMAX);
 #pragma unroll
-        for (int q = 0; q < NMAX; ++q) dst[q] = yacc.get(q);
+            for (int q = 0; q < NMAX; q += 2) {
+                const float2 u = yacc.get(q), v = yacc.get(q + 1);
+                dst[q / 2] = make_float4(u.x, u.y, v.x, v.y);
+            }
+        }
     }
+#ifdef CELES_TRACE
+    if (tid == 0 && blockIdx.x < 8192) {
+        unsigned long long t1; unsigned smid;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1));
+        asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+        g_trace[3 * blockIdx.x] = smid; g_trace[3 * blockIdx.x + 1] = trace_t0; g_trace[3 * blockIdx.x + 2] = t1;
+    }
+#endif
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// H8-H9: sums the emitter splits and returns to the (tau, l, m) basis; if tdiag != nullptr the epilogue of
-// eq. (9) is fused: out = b - T y with T the diagonal Q^i_{tau,l} expanded to [N][nmax].
+// H8-H9: for the receivers [row_begin, row_end) sums the partial-sum slots of each receiver block in slot order and
+// returns to the (tau, l, m) basis; if tdiag != nullptr the epilogue of eq. (9) is fused: out = b - T y with T the
+// diagonal Q^i_{tau,l} expanded to [N][nmax].  out holds rows row_begin.. only ([row_end - row_begin][nmax]); b and
+// tdiag are the full [N][nmax] arrays.
 //   DIRECT : y_1 = (y_+ + y_-)/2, y_2 = (y_+ - y_-)/2.
 //   ROTATED: inverse of the orthonormal transform of pack_kernel.  One thread per (sphere, (l,m)).
 template <int VARIANT>
-__global__ void finalize_kernel(int N, int H, int splits, const float2* __restrict__ ypart,
-                                const float2* __restrict__ tdiag, const float2* __restrict__ b,
-                                float2* __restrict__ out) {
+__global__ void finalize_kernel(int row_begin, int row_end, int H, int bs, const int* __restrict__ slot_begin,
+                                const float2* __restrict__ ypart, const float2* __restrict__ tdiag,
+                                const float2* __restrict__ b, float2* __restrict__ out) {
     constexpr bool ROTATED = VARIANT != kDirect;
     const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (t >= (long long)N * H) return;
-    const long long i = t / H;
-    const int q = (int)(t - i * H);
-    const size_t stride = (size_t)N * 2 * H;
+    if (t >= (long long)(row_end - row_begin) * H) return;
+    const long long i = row_begin + t / H;
+    const int q = (int)(t - (i - row_begin) * H);
+    const int rblock = (int)(i / bs);
+    const int s0 = slot_begin[rblock], s1 = slot_begin[rblock + 1];
+    const size_t stride = (size_t)kBlock * 2 * H;                  // one slot
+    const float2* y0 = ypart + (size_t)(i - (long long)rblock * bs) * 2 * H;
     float2 y1, y2;
     if (!ROTATED) {
         float pr = 0.f, pi = 0.f, mr = 0.f, mi = 0.f;
-        for (int s = 0; s < splits; ++s) {
-            const float2 yp = ypart[s * stride + i * 2 * H + q], ym = ypart[s * stride + i * 2 * H + H + q];
+        for (int s = s0; s < s1; ++s) {
+            const float2 yp = y0[s * stride + q], ym = y0[s * stride + H + q];
             pr += yp.x; pi += yp.y; mr += ym.x; mi += ym.y;
         }
         y1 = make_float2(0.5f * (pr + mr), 0.5f * (pi + mi));
@@ -209,8 +262,8 @@ __global__ void finalize_kernel(int N, int H, int splits, const float2* __restri
         const int qa = base + (am ? 2 * am - 1 : 0);         // u+_|m| (or u_0)
         const int qb = base + 2 * am;                        // u-_|m| (unused for m = 0)
         float sar = 0.f, sai = 0.f, sbr = 0.f, sbi = 0.f, aar = 0.f, aai = 0.f, abr = 0.f, abi = 0.f;
-        for (int s = 0; s < splits; ++s) {
-            const float2* y = ypart + s * stride + i * 2 * H;
+        for (int s = s0; s < s1; ++s) {
+            const float2* y = y0 + s * stride;
             const float2 sa = y[qa], aa = y[H + qa];
             sar += sa.x; sai += sa.y; aar += aa.x; aai += aa.y;
             if (am) {
@@ -240,8 +293,9 @@ __global__ void finalize_kernel(int N, int H, int splits, const float2* __restri
         y1 = make_float2(b1.x - (t1.x * y1.x - t1.y * y1.y), b1.y - (t1.x * y1.y + t1.y * y1.x));
         y2 = make_float2(b2.x - (t2.x * y2.x - t2.y * y2.y), b2.y - (t2.x * y2.y + t2.y * y2.x));
     }
-    out[o1] = y1;
-    out[o2] = y2;
+    const size_t r1 = o1 - (size_t)row_begin * 2 * H;
+    out[r1] = y1;
+    out[r1 + H] = y2;
 }
 
 }  // namespace celes

@@ -4,6 +4,7 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include <new>
 #include <vector>
 
 #include "../../include/celes.h"
@@ -14,7 +15,16 @@ struct celes_ctx {
     int N = 0, lmax = 0, nmax = 0;
     double k = 0.0;
     int device = 0, sm_count = 0;
-    int rblocks = 0, splits = 1, chunk = 0, etile = 32;
+    int etile = 32;
+    // work partition of the coupling kernel (work_partition.h): receiver blocks of bs spheres, n_cta CTAs walking
+    // n_seg segments, one partial-sum slot per segment
+    int bs = 0, rblocks = 0, n_cta = 0, n_seg = 0, fixed_splits = 0;
+    int* cta_begin = nullptr;    // [n_cta + 1]
+    int4* seg = nullptr;         // [n_seg] (rblock, e_begin, e_end, slot)
+    int* slot_begin = nullptr;   // [rblocks + 1]
+    std::vector<int> h_cta_of_block_first, h_cta_of_block_last;   // [rblocks] first / last CTA with a segment of the block
+    bool extended_range = false; // kd carried as FP32 + residual (pair_math.cuh, EXT); chosen by celes_setup
+    double kd_max = 0.0;         // k x diagonal of the centres' bounding box
     int variant = celes::kRotated;   // CELES_TRANSLATION_*: packed rotated (default), direct sum, scalar rotated
     size_t coupling_smem = 0;
     std::vector<double> pos;     // host copy of the centres [N][3] (partition of the preconditioner)
@@ -23,7 +33,9 @@ struct celes_ctx {
     float4* htab = nullptr;      // Hankel lookup table [nodes][2 lmax + 1] (CELES_HANKEL_TABLE), else null
     HankelTable htab_desc = {nullptr, 0.0f, 0.0f, 0};
     float2* bpm = nullptr;       // [N][nmax] work: [b_+ | b_-]
-    float2* ypart = nullptr;     // [splits][N][nmax] work: partial sums of the emitter splits
+    float2* ypart = nullptr;     // [n_seg][kBlock][nmax] work: partial sums, one slot per segment
+    void* scratch = nullptr;     // device scratch of the field calls (direction / beam / point tables), grown on demand
+    size_t scratch_bytes = 0;
     float2 *host_in = nullptr, *host_out = nullptr;   // [N][nmax] staging of the *_host entry points (allocated on first use)
     // Krylov work space (allocated on the first celes_solve)
     int kry_restart = 0, dot_blocks = 0;
@@ -56,10 +68,20 @@ struct celes_ctx {
         }                                             \
     } while (0)
 
+// Nothing may throw across the C ABI (celes.h): every extern "C" body that allocates host memory runs inside this.
+#define CELES_NOTHROW(call)                                  \
+    try { return (call); }                                   \
+    catch (const std::bad_alloc&) { return CELES_ENOMEM; }   \
+    catch (...) { return CELES_ECUDA; }
+
 namespace celes {
 namespace host {
-// y = W b (system == false) or out = b - T (W b): pack -> coupling -> finalize, all on stream s (celes.cu)
-int run_matvec(celes_ctx* c, const float2* b, float2* out, bool system, cudaStream_t s);
+// rows [row_begin, row_end) of y = W b (system == false) or out = b - T (W b): pack -> coupling -> finalize, all on
+// stream s; b is the full vector, out holds the rows only (celes.cu)
+int run_matvec(celes_ctx* c, const float2* b, float2* out, bool system, cudaStream_t s, int row_begin, int row_end);
+inline int run_matvec(celes_ctx* c, const float2* b, float2* out, bool system, cudaStream_t s) {
+    return run_matvec(c, b, out, system, s, 0, c->N);
+}
 // z = blockdiag(M_j^{-1}) v, and release of the preconditioner (precond.cu)
 int precond_apply(celes_ctx* c, const float2* v, float2* z, cudaStream_t s);
 void free_precond(celes_ctx* c);

@@ -12,6 +12,33 @@
 #include "gaussian_beam.cuh"
 #include "near_field.cuh"
 
+namespace {
+
+// Device scratch of the field calls, kept with the context: grows when a call needs more (the only time these calls
+// synchronise the stream and touch the allocator), is reused otherwise.  Pieces are carved at 256-byte boundaries.
+struct Scratch {
+    celes_ctx* ctx;
+    size_t used = 0;
+    explicit Scratch(celes_ctx* c) : ctx(c) {}
+    static size_t align(size_t b) { return (b + 255) & ~(size_t)255; }
+    int reserve(size_t total, cudaStream_t s) {
+        if (total <= ctx->scratch_bytes) return CELES_OK;
+        if (cudaStreamSynchronize(s) != cudaSuccess) return CELES_ECUDA;      // earlier calls may still read the old block
+        cudaFree(ctx->scratch);
+        ctx->scratch = nullptr; ctx->scratch_bytes = 0;
+        if (cudaMalloc(&ctx->scratch, total) != cudaSuccess) { cudaGetLastError(); return CELES_ENOMEM; }
+        ctx->scratch_bytes = total;
+        return CELES_OK;
+    }
+    template <class T> T* take(size_t count) {
+        T* p = reinterpret_cast<T*>(static_cast<char*>(ctx->scratch) + used);
+        used += align(sizeof(T) * count);
+        return p;
+    }
+};
+
+}  // namespace
+
 extern "C" {
 
 int celes_far_field(celes_ctx* ctx, const void* b_dev, int n_dir, const double* alpha, const double* beta, void* g_dev,
@@ -25,13 +52,14 @@ int celes_far_field(celes_ctx* ctx, const void* b_dev, int n_dir, const double* 
     int splits = std::max(1, std::min((8 * ctx->sm_count + gx - 1) / gx, std::max(1, ctx->N / (4 * celes::kFarTile))));
     const int chunk = ((ctx->N + splits - 1) / splits + celes::kFarTile - 1) / celes::kFarTile * celes::kFarTile;
     splits = (ctx->N + chunk - 1) / chunk;
-    double *d_ang = nullptr, *d_dir = nullptr;
-    float2 *d_coef = nullptr, *d_part = nullptr;
-    int rc = CELES_OK;
-    if (cudaMalloc(&d_ang, sizeof(double) * 2 * (size_t)n_dir) != cudaSuccess ||
-        cudaMalloc(&d_dir, sizeof(double) * 3 * (size_t)n_dir) != cudaSuccess ||
-        cudaMalloc(&d_coef, sizeof(float2) * (size_t)rows * nmax) != cudaSuccess ||
-        cudaMalloc(&d_part, sizeof(float2) * (size_t)rows * splits) != cudaSuccess) rc = CELES_ENOMEM;
+    Scratch sc(ctx);
+    int rc = sc.reserve(Scratch::align(sizeof(double) * 2 * (size_t)n_dir) + Scratch::align(sizeof(double) * 3 * (size_t)n_dir) +
+                        Scratch::align(sizeof(float2) * (size_t)rows * nmax) + Scratch::align(sizeof(float2) * (size_t)rows * splits), s);
+    if (rc) return rc;
+    double* d_ang = sc.take<double>(2 * (size_t)n_dir);
+    double* d_dir = sc.take<double>(3 * (size_t)n_dir);
+    float2* d_coef = sc.take<float2>((size_t)rows * nmax);
+    float2* d_part = sc.take<float2>((size_t)rows * splits);
     if (!rc && (cudaMemcpyAsync(d_ang, alpha, sizeof(double) * n_dir, cudaMemcpyHostToDevice, s) != cudaSuccess ||
                 cudaMemcpyAsync(d_ang + n_dir, beta, sizeof(double) * n_dir, cudaMemcpyHostToDevice, s) != cudaSuccess)) rc = CELES_ECUDA;
     if (!rc) {
@@ -49,8 +77,6 @@ int celes_far_field(celes_ctx* ctx, const void* b_dev, int n_dir, const double* 
         if (!rc) celes::far_field_reduce_kernel<<<(rows + 255) / 256, 256, 0, s>>>(rows, splits, d_part, (float2*)g_dev);
         if (!rc && cudaGetLastError() != cudaSuccess) rc = CELES_ECUDA;
     }
-    if (cudaStreamSynchronize(s) != cudaSuccess && !rc) rc = CELES_ECUDA;
-    cudaFree(d_ang); cudaFree(d_dir); cudaFree(d_coef); cudaFree(d_part);
     return rc;
 }
 
@@ -64,7 +90,7 @@ int celes_plane_wave(celes_ctx* ctx, double alpha, double beta, int polarisation
     return cudaGetLastError() == cudaSuccess ? CELES_OK : CELES_ECUDA;
 }
 
-int celes_gaussian_beam(celes_ctx* ctx, const celes_beam* beam, void* a_in_dev, void* cuda_stream) {
+static int gaussian_beam_impl(celes_ctx* ctx, const celes_beam* beam, void* a_in_dev, void* cuda_stream) {
     if (!ctx || !beam || !a_in_dev) return CELES_EINVAL;
     const int n_beta = beam->n_beta > 0 ? beam->n_beta : 400;
     if (!(beam->waist > 0.0) || !std::isfinite(beam->waist) || n_beta > 100000) return CELES_EINVAL;
@@ -74,12 +100,14 @@ int celes_gaussian_beam(celes_ctx* ctx, const celes_beam* beam, void* a_in_dev, 
     std::vector<double> sb, cb;
     std::vector<double2> cminus, cplus;
     celes::gaussian_beam_tables(ctx->lmax, n_beta, ctx->k, beam->waist, sb, cb, cminus, cplus);
-    double *d_sb = nullptr, *d_cb = nullptr;
-    double2 *d_cm = nullptr, *d_cp = nullptr;
-    int rc = CELES_OK;
-    if (cudaMalloc(&d_sb, sizeof(double) * n_beta) != cudaSuccess || cudaMalloc(&d_cb, sizeof(double) * n_beta) != cudaSuccess ||
-        cudaMalloc(&d_cm, sizeof(double2) * cminus.size()) != cudaSuccess ||
-        cudaMalloc(&d_cp, sizeof(double2) * cplus.size()) != cudaSuccess) rc = CELES_ENOMEM;
+    Scratch sc(ctx);
+    int rc = sc.reserve(2 * Scratch::align(sizeof(double) * n_beta) + Scratch::align(sizeof(double2) * cminus.size()) +
+                        Scratch::align(sizeof(double2) * cplus.size()), s);
+    if (rc) return rc;
+    double* d_sb = sc.take<double>(n_beta);
+    double* d_cb = sc.take<double>(n_beta);
+    double2* d_cm = sc.take<double2>(cminus.size());
+    double2* d_cp = sc.take<double2>(cplus.size());
     if (!rc && (cudaMemcpyAsync(d_sb, sb.data(), sizeof(double) * n_beta, cudaMemcpyHostToDevice, s) != cudaSuccess ||
                 cudaMemcpyAsync(d_cb, cb.data(), sizeof(double) * n_beta, cudaMemcpyHostToDevice, s) != cudaSuccess ||
                 cudaMemcpyAsync(d_cm, cminus.data(), sizeof(double2) * cminus.size(), cudaMemcpyHostToDevice, s) != cudaSuccess ||
@@ -91,20 +119,23 @@ int celes_gaussian_beam(celes_ctx* ctx, const celes_beam* beam, void* a_in_dev, 
             beam->alpha_G, make_double2(beam->E0_re, beam->E0_im), d_sb, d_cb, d_cm, d_cp, (float2*)a_in_dev);
         if (cudaGetLastError() != cudaSuccess) rc = CELES_ECUDA;
     }
-    if (cudaStreamSynchronize(s) != cudaSuccess && !rc) rc = CELES_ECUDA;
-    cudaFree(d_sb); cudaFree(d_cb); cudaFree(d_cm); cudaFree(d_cp);
     return rc;
 }
 
-int celes_scattered_field(celes_ctx* ctx, const void* b_dev, int n_pts, const double* pts_xyz, void* e_dev, void* cuda_stream) {
+int celes_gaussian_beam(celes_ctx* ctx, const celes_beam* beam, void* a_in_dev, void* cuda_stream) {
+    CELES_NOTHROW(gaussian_beam_impl(ctx, beam, a_in_dev, cuda_stream))
+}
+
+static int scattered_field_impl(celes_ctx* ctx, const void* b_dev, int n_pts, const double* pts_xyz, void* e_dev, void* cuda_stream) {
     if (!ctx || !b_dev || !e_dev || !pts_xyz || n_pts < 1) return CELES_EINVAL;
     for (long long t = 0; t < 3LL * n_pts; ++t) if (!std::isfinite(pts_xyz[t])) return CELES_EINVAL;
     cudaStream_t s = (cudaStream_t)cuda_stream;
     std::vector<double> kp(3 * (size_t)n_pts);
     for (size_t t = 0; t < kp.size(); ++t) kp[t] = ctx->k * pts_xyz[t];
-    double* d_pts = nullptr;
-    CU_TRY(cudaMalloc(&d_pts, sizeof(double) * kp.size()));
-    int rc = CELES_OK;
+    Scratch sc(ctx);
+    int rc = sc.reserve(Scratch::align(sizeof(double) * kp.size()), s);
+    if (rc) return rc;
+    double* d_pts = sc.take<double>(kp.size());
     if (cudaMemcpyAsync(d_pts, kp.data(), sizeof(double) * kp.size(), cudaMemcpyHostToDevice, s) != cudaSuccess) rc = CELES_ECUDA;
     if (!rc) {
         const int grid = (n_pts + celes::kNearThreads - 1) / celes::kNearThreads;
@@ -120,9 +151,11 @@ int celes_scattered_field(celes_ctx* ctx, const void* b_dev, int n_pts, const do
         }
         if (!rc && cudaGetLastError() != cudaSuccess) rc = CELES_ECUDA;
     }
-    if (cudaStreamSynchronize(s) != cudaSuccess && !rc) rc = CELES_ECUDA;
-    cudaFree(d_pts);
     return rc;
+}
+
+int celes_scattered_field(celes_ctx* ctx, const void* b_dev, int n_pts, const double* pts_xyz, void* e_dev, void* cuda_stream) {
+    CELES_NOTHROW(scattered_field_impl(ctx, b_dev, n_pts, pts_xyz, e_dev, cuda_stream))
 }
 
 }  // extern "C"

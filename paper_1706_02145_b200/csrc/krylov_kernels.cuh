@@ -93,9 +93,8 @@ __global__ void multi_axpy_kernel(long long n, int k, double alpha, const double
     }
 }
 
-// out = w / sqrt(nrm2[0].x)   (nrm2 = <w,w> from the dot kernels); out may alias w
-__global__ void scale_by_inv_norm_kernel(long long n, const double2* __restrict__ nrm2, const float2* __restrict__ w,
-                                         float2* __restrict__ out) {
+// out = w / sqrt(nrm2[0].x)   (nrm2 = <w,w> from the dot kernels); out may alias w (so neither is __restrict__)
+__global__ void scale_by_inv_norm_kernel(long long n, const double2* __restrict__ nrm2, const float2* w, float2* out) {
     const double s = nrm2[0].x > 0.0 ? rsqrt(nrm2[0].x) : 0.0;
     for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += (long long)gridDim.x * blockDim.x) {
         const float2 v = w[t];
@@ -111,8 +110,8 @@ __global__ void sub_kernel(long long n, const float2* __restrict__ a, const floa
 
 // out = a x + b y + c z  (complex scalars by value; y, z may be nullptr when their scalar is unused; out may alias
 // any input).  The vector updates of BiCGSTAB.
-__global__ void lincomb_kernel(long long n, double2 a, const float2* __restrict__ x, double2 b, const float2* y,
-                               double2 c, const float2* z, float2* out) {
+__global__ void lincomb_kernel(long long n, double2 a, const float2* x, double2 b, const float2* y, double2 c,
+                               const float2* z, float2* out) {
     for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += (long long)gridDim.x * blockDim.x) {
         const float2 xv = x[t];
         double r = a.x * xv.x - a.y * xv.y, i = a.x * xv.y + a.y * xv.x;

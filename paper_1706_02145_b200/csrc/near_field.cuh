@@ -54,7 +54,7 @@ __global__ void __launch_bounds__(kNearThreads) near_field_kernel(int N, int n_p
             const float st = rho2 * rhoinv * rinv;
             // h_l(x), l = 0..LMAX
             float sx, cx;
-            sincos_kd(x, &sx, &cx);
+            sincos_kd(x, 0.0f, &sx, &cx);
             float2 h[LMAX + 1];
             h[0] = make_float2(sx * rinv, -cx * rinv);
             h[1] = make_float2(fmaf(sx, rinv, -cx) * rinv, -fmaf(cx, rinv, sx) * rinv);

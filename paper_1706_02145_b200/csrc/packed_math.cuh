@@ -35,13 +35,15 @@ CELES_DEVICE float2 cmul2(float2 k, float2 x) {
 // useless on their own; after a Cody-Waite reduction to [-pi, pi] (2 pi = 6.28125 + 1.9353072e-3: the first product
 // n * 6.28125 is exact for n < 2^15) their absolute error is ~4e-7, far inside the 1e-4 budget, and the pair saves the
 // ~25 instructions of sincosf's polynomial path.  Define CELES_ACCURATE_SINCOS to get sincosf back.
-CELES_DEVICE void sincos_kd(float x, float* s, float* c) {
+// x_lo: the part of kd that FP32 x does not hold (0 in the standard range mode); it is added AFTER the reduction,
+// where it is not absorbed by the rounding of x.
+CELES_DEVICE void sincos_kd(float x, float x_lo, float* s, float* c) {
 #ifdef CELES_ACCURATE_SINCOS
-    sincosf(x, s, c);
+    sincosf(x + x_lo, s, c);
 #else
     const float n = rintf(x * 0.15915494309189535f);
     float r = fmaf(n, -6.28125f, x);
-    r = fmaf(n, -1.9353071795864769e-3f, r);
+    r = fmaf(n, -1.9353071795864769e-3f, r) + x_lo;
     __sincosf(r, s, c);
 #endif
 }

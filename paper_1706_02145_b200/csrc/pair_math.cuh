@@ -28,12 +28,17 @@ struct PairBodyPk;    // packed (FFMA2) rotate / axial-translate / rotate varian
 #include "generated/coupling_pk_lmax5.inc"
 
 
-// dx, dy, dz: components of k (r_i - r_i') (dimensionless), already rounded to FP32 AFTER the subtraction
-// was done in FP64 (coordinate rounding is the dominant FP32 error otherwise).
+// ddx, ddy, ddz: components of k (r_i - r_i') (dimensionless) from the FP64 subtraction; they are rounded to FP32
+// here, AFTER the subtraction (coordinate rounding is the dominant FP32 error otherwise).
+// EXT (extended range): kd itself rounded to FP32 carries a phase error of kd 2^-24 rad, which reaches the 1e-4 budget
+// for clusters a few thousand wavelengths across.  EXT recovers the lost part with one Newton residual in FP64,
+// kd = x + (|dd|^2 - x^2) / (2 x), and hands it to the argument reduction of e^{ikd} (six FP64-pipe instructions per
+// pair; everything else is unchanged).  celes_setup switches it on by the extent of the cluster.
 // bload(q): emitter coefficient q in the variant's work basis;  yacc: accumulator policy of the receiver.
-template <int LMAX, int VARIANT, bool TABLE, class BLoad, class YAcc>
-CELES_DEVICE void pair_translate(float dx, float dy, float dz, const HankelTable& htab, const BLoad& bload, YAcc& yacc) {
+template <int LMAX, int VARIANT, bool TABLE, bool EXT = false, class BLoad, class YAcc>
+CELES_DEVICE void pair_translate(double ddx, double ddy, double ddz, const HankelTable& htab, const BLoad& bload, YAcc& yacc) {
     constexpr int P = 2 * LMAX + 1;
+    const float dx = (float)ddx, dy = (float)ddy, dz = (float)ddz;
     // ---- H2 geometry: spherical coordinates of d
     const float rho2 = fmaf(dx, dx, dy * dy);
     const float r2 = fmaf(dz, dz, rho2);
@@ -63,8 +68,12 @@ CELES_DEVICE void pair_translate(float dx, float dy, float dz, const HankelTable
         PairBodyPk<LMAX>::run(h, ct, st, cph, sph, bload, yacc);
         return;
     }
-    float sx, cx;
-    sincos_kd(x, &sx, &cx);                          // kd reaches ~1000 rad: reduced first
+    float sx, cx, x_lo = 0.0f;
+    if constexpr (EXT) {
+        const double xd = (double)x;
+        x_lo = (float)fma(-xd, xd, fma(ddx, ddx, fma(ddy, ddy, ddz * ddz))) * (0.5f * rinv);
+    }
+    sincos_kd(x, x_lo, &sx, &cx);                    // kd reaches ~1000 rad and more: reduced first
     if constexpr (VARIANT == celes::kRotated) {             // the same recurrence on packed (Re, Im)
         float2 h[P];
         h[0] = mul2(bc2(rinv), make_float2(sx, -cx));

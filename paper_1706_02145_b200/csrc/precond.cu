@@ -34,13 +34,17 @@ using celes::host::precond_apply;
 
 extern "C" {
 
-int celes_partition(int N, const double* pos_xyz, const double* edge_xyz, int* group_of, int* n_groups) {
+static int partition_impl(int N, const double* pos_xyz, const double* edge_xyz, int* group_of, int* n_groups) {
     if (N < 1 || !pos_xyz || !edge_xyz || !group_of) return CELES_EINVAL;
     celes::Partition part;
     if (!celes::build_partition(N, pos_xyz, edge_xyz, part)) return CELES_EINVAL;
     std::memcpy(group_of, part.group_of.data(), sizeof(int) * (size_t)N);
     if (n_groups) *n_groups = part.n_groups();
     return CELES_OK;
+}
+
+int celes_partition(int N, const double* pos_xyz, const double* edge_xyz, int* group_of, int* n_groups) {
+    CELES_NOTHROW(partition_impl(N, pos_xyz, edge_xyz, group_of, n_groups))
 }
 
 // Block-diagonal preconditioner: (1) cuboid partition, (2) blocks M_j = 1 - T W on the device,

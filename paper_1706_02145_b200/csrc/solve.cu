@@ -26,22 +26,26 @@ void celes::host::free_krylov(celes_ctx* c) {
 
 namespace {
 
+// Work space of the solvers, sized for `restart`.  All or nothing: a failed (re-)allocation releases everything and
+// leaves kry_restart = 0, so a later call can never run on a half-allocated work space.
 int ensure_krylov(celes_ctx* c, int restart) {
     if (c->V && c->kry_restart >= restart) return CELES_OK;
-    cudaFree(c->V); cudaFree(c->rhs); cudaFree(c->tmp); cudaFree(c->partial); cudaFree(c->coef); cudaFree(c->hsum);
-    if (c->hhost) cudaFreeHost(c->hhost);
-    c->V = nullptr; c->rhs = c->tmp = nullptr; c->partial = c->coef = c->hsum = nullptr; c->hhost = nullptr;
+    celes::host::free_krylov(c);
     const size_t n = (size_t)c->N * c->nmax;
     c->dot_blocks = (int)std::min<size_t>((n + celes::kDotBlock - 1) / celes::kDotBlock, (size_t)c->sm_count * 4);
-    CU_TRY(cudaMalloc(&c->V, sizeof(float2) * n * (restart + 1)));
-    CU_TRY(cudaMalloc(&c->rhs, sizeof(float2) * n));
-    CU_TRY(cudaMalloc(&c->tmp, sizeof(float2) * n));
-    CU_TRY(cudaMalloc(&c->partial, sizeof(double2) * c->dot_blocks * (restart + 1)));
-    CU_TRY(cudaMalloc(&c->coef, sizeof(double2) * (restart + 2)));
-    CU_TRY(cudaMalloc(&c->hsum, sizeof(double2) * 2 * (restart + 2)));
-    CU_TRY(cudaMallocHost(&c->hhost, sizeof(double2) * 3 * (restart + 2)));
-    for (int q = 0; q < 2; ++q)
-        if (!c->kry_ev[q]) CU_TRY(cudaEventCreateWithFlags(&c->kry_ev[q], cudaEventDisableTiming));
+    cudaError_t e = cudaMalloc(&c->V, sizeof(float2) * n * (restart + 1));
+    if (e == cudaSuccess) e = cudaMalloc(&c->rhs, sizeof(float2) * n);
+    if (e == cudaSuccess) e = cudaMalloc(&c->tmp, sizeof(float2) * n);
+    if (e == cudaSuccess) e = cudaMalloc(&c->partial, sizeof(double2) * c->dot_blocks * (restart + 1));
+    if (e == cudaSuccess) e = cudaMalloc(&c->coef, sizeof(double2) * (restart + 2));
+    if (e == cudaSuccess) e = cudaMalloc(&c->hsum, sizeof(double2) * 2 * (restart + 2));
+    if (e == cudaSuccess) e = cudaMallocHost(&c->hhost, sizeof(double2) * 3 * (restart + 2));
+    for (int q = 0; q < 2 && e == cudaSuccess; ++q) e = cudaEventCreateWithFlags(&c->kry_ev[q], cudaEventDisableTiming);
+    if (e != cudaSuccess) {
+        celes::host::free_krylov(c);
+        cudaGetLastError();
+        return e == cudaErrorMemoryAllocation ? CELES_ENOMEM : CELES_ECUDA;
+    }
     c->kry_restart = restart;
     return CELES_OK;
 }
@@ -167,8 +171,8 @@ extern "C" {
 // iteration brings the Hessenberg column to the host, where Givens rotations track the residual estimate; the
 // device work of the next column is enqueued before the host waits for that copy (one column of look-ahead).
 // The TRUE residual is recomputed at every restart and decides convergence (reading R14).
-int celes_solve(celes_ctx* ctx, const void* a_in_dev, void* x_dev, const celes_solve_opts* o, celes_solve_info* info,
-                void* cuda_stream) {
+static int solve_impl(celes_ctx* ctx, const void* a_in_dev, void* x_dev, const celes_solve_opts* o, celes_solve_info* info,
+                      void* cuda_stream) {
     if (!ctx || !a_in_dev || !x_dev) return CELES_EINVAL;
     const int method = o ? o->method : CELES_GMRES;
     const int restart = (o && o->restart > 0) ? o->restart : 30;
@@ -180,6 +184,7 @@ int celes_solve(celes_ctx* ctx, const void* a_in_dev, void* x_dev, const celes_s
     if (pc && !ctx->pc_ready) return CELES_EINVAL;            // celes_precond_setup first
     cudaStream_t s = (cudaStream_t)cuda_stream;
     const auto t_start = std::chrono::steady_clock::now();
+    if (info) std::memset(info, 0, sizeof(*info));
     int rc = ensure_krylov(ctx, method == CELES_BICGSTAB ? std::max(restart, 8) : restart);
     if (rc) return rc;
     const long long n = (long long)ctx->N * ctx->nmax;
@@ -190,7 +195,6 @@ int celes_solve(celes_ctx* ctx, const void* a_in_dev, void* x_dev, const celes_s
 
     int iterations = 0, matvecs = 0, n_hist = 0, converged = 0;
     double rel = 0.0;
-    if (info) std::memset(info, 0, sizeof(*info));
     auto push_hist = [&](double v) { if (info && n_hist < CELES_MAX_HISTORY) info->history[n_hist++] = v; };
     auto finish = [&](int code) {
         if (info) {
@@ -201,14 +205,19 @@ int celes_solve(celes_ctx* ctx, const void* a_in_dev, void* x_dev, const celes_s
         return code;
     };
 
+#define SOLVE_TRY(expr)                                                                          \
+    do {                                                                                         \
+        cudaError_t e_ = (expr);                                                                 \
+        if (e_ != cudaSuccess) return finish(e_ == cudaErrorMemoryAllocation ? CELES_ENOMEM : CELES_ECUDA); \
+    } while (0)
     // rhs = T a_in (eq. 8)
     celes::tapply_kernel<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(n, ctx->tdiag, (const float2*)a_in_dev, ctx->rhs);
     double fnorm = 0.0;
     rc = device_norm(ctx, n, ctx->rhs, &fnorm, s);
     if (rc) return finish(rc);
     if (fnorm == 0.0) {                       // zero right-hand side: x = 0
-        CU_TRY(cudaMemsetAsync(x, 0, sizeof(float2) * n, s));
-        CU_TRY(cudaStreamSynchronize(s));
+        SOLVE_TRY(cudaMemsetAsync(x, 0, sizeof(float2) * n, s));
+        SOLVE_TRY(cudaStreamSynchronize(s));
         converged = 1;
         return finish(CELES_OK);
     }
@@ -253,7 +262,7 @@ int celes_solve(celes_ctx* ctx, const void* a_in_dev, void* x_dev, const celes_s
             }
             if (r2) return r2;
             ++matvecs;
-            CU_TRY(cudaMemsetAsync(hsum, 0, sizeof(double2) * (jc + 2), s));
+            SOLVE_TRY(cudaMemsetAsync(hsum, 0, sizeof(double2) * (jc + 2), s));
             for (int pass = 0; pass < 2; ++pass) {
                 r2 = device_dots(ctx, n, jc + 1, V, w, ctx->coef, hsum, s);
                 if (r2) return r2;
@@ -263,8 +272,8 @@ int celes_solve(celes_ctx* ctx, const void* a_in_dev, void* x_dev, const celes_s
             r2 = device_dots(ctx, n, 1, w, w, hsum + (jc + 1), nullptr, s);
             if (r2) return r2;
             celes::scale_by_inv_norm_kernel<<<eb, 256, 0, s>>>(n, hsum + (jc + 1), w, w);
-            CU_TRY(cudaMemcpyAsync(ctx->hhost + (size_t)(jc & 1) * hs, hsum, sizeof(double2) * (jc + 2), cudaMemcpyDeviceToHost, s));
-            CU_TRY(cudaEventRecord(ctx->kry_ev[jc & 1], s));
+            SOLVE_TRY(cudaMemcpyAsync(ctx->hhost + (size_t)(jc & 1) * hs, hsum, sizeof(double2) * (jc + 2), cudaMemcpyDeviceToHost, s));
+            SOLVE_TRY(cudaEventRecord(ctx->kry_ev[jc & 1], s));
             return CELES_OK;
         };
         int j = 0, enq = 0;
@@ -279,7 +288,7 @@ int celes_solve(celes_ctx* ctx, const void* a_in_dev, void* x_dev, const celes_s
                 if (rc) return finish(rc);
                 ++enq;
             }
-            CU_TRY(cudaEventSynchronize(ctx->kry_ev[j & 1]));
+            SOLVE_TRY(cudaEventSynchronize(ctx->kry_ev[j & 1]));
             ++iterations;
             const double2* hh = ctx->hhost + (size_t)(j & 1) * hs;
             // Hessenberg column j, Givens rotations
@@ -312,9 +321,9 @@ int celes_solve(celes_ctx* ctx, const void* a_in_dev, void* x_dev, const celes_s
             yv[i] = acc / Hm[(size_t)i * (restart + 1) + i];
         }
         for (int i = 0; i < j; ++i) hup[i] = make_double2(yv[i].real(), yv[i].imag());
-        CU_TRY(cudaMemcpyAsync(ctx->coef, hup, sizeof(double2) * j, cudaMemcpyHostToDevice, s));
+        SOLVE_TRY(cudaMemcpyAsync(ctx->coef, hup, sizeof(double2) * j, cudaMemcpyHostToDevice, s));
         if (j > 0 && pc) {                                     // x += P^{-1} (V y)
-            CU_TRY(cudaMemsetAsync(ctx->tmp, 0, sizeof(float2) * n, s));
+            SOLVE_TRY(cudaMemsetAsync(ctx->tmp, 0, sizeof(float2) * n, s));
             rc = device_axpys(ctx, n, j, 1.0, ctx->coef, V, ctx->tmp, s);
             if (rc) return finish(rc);
             rc = precond_apply(ctx, ctx->tmp, ctx->pc_tmp, s);
@@ -324,8 +333,14 @@ int celes_solve(celes_ctx* ctx, const void* a_in_dev, void* x_dev, const celes_s
             rc = device_axpys(ctx, n, j, 1.0, ctx->coef, V, x, s);
             if (rc) return finish(rc);
         }
-        CU_TRY(cudaStreamSynchronize(s));      // hhost is reused by the next cycle
+        SOLVE_TRY(cudaStreamSynchronize(s));      // hhost is reused by the next cycle
     }
+#undef SOLVE_TRY
+}
+
+int celes_solve(celes_ctx* ctx, const void* a_in_dev, void* x_dev, const celes_solve_opts* o, celes_solve_info* info,
+                void* cuda_stream) {
+    CELES_NOTHROW(solve_impl(ctx, a_in_dev, x_dev, o, info, cuda_stream))
 }
 
 }  // extern "C"

@@ -37,8 +37,18 @@ def cuobjdump() -> str | None:
     return shutil.which("cuobjdump") or ("/usr/local/cuda/bin/cuobjdump" if os.path.exists("/usr/local/cuda/bin/cuobjdump") else None)
 
 
-def coupling_symbol(lmax: int, variant: int = 0, table: bool = False) -> str:
-    return f"_ZN5celes15coupling_kernelILi{lmax}ELi{variant}ELb{int(table)}EEEviii11HankelTablePKdPK6float2PS4_"
+def coupling_symbol(lmax: int, variant: int = 0, table: bool = False, extended: bool = False, lib: str = LIB) -> str:
+    """Mangled name of coupling_kernel<lmax, variant, table, extended>, looked up in the library's symbol table (the
+    argument list is part of the name, so it is not spelled out here)."""
+    exe = cuobjdump()
+    if exe is None:
+        raise RuntimeError("cuobjdump not found")
+    prefix = f"_ZN5celes15coupling_kernelILi{lmax}ELi{variant}ELb{int(table)}ELb{int(extended)}EEE"
+    out = subprocess.run([exe, "-symbols", lib], capture_output=True, text=True, check=False).stdout
+    for tok in out.split():
+        if tok.startswith(prefix):
+            return tok
+    raise RuntimeError(f"no symbol {prefix}* in {lib}")
 
 
 def dump(symbol: str, lib: str = LIB) -> str:
@@ -98,8 +108,8 @@ def count_kernel(symbol: str, lib: str = LIB) -> dict:
             "flops_per_pair": flops, "lane_ops_per_pair": lane}
 
 
-def coupling_counts(lmax: int, translation: str = "rotated", table: bool = False, lib: str = LIB) -> dict:
-    return count_kernel(coupling_symbol(lmax, VARIANTS[translation], table), lib)
+def coupling_counts(lmax: int, translation: str = "rotated", table: bool = False, extended: bool = False, lib: str = LIB) -> dict:
+    return count_kernel(coupling_symbol(lmax, VARIANTS[translation], table, extended, lib), lib)
 
 
 def committed() -> dict:

@@ -23,9 +23,11 @@ def _built():
 
 
 def test_library_exports_every_declared_symbol():
-    hdr = open(os.path.join(ROOT, "include", "celes.h")).read()
-    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
-    declared = set(re.findall(r"\b(celes_[a-z0-9_]+)\s*\(", hdr))
+    declared = set()
+    for name in os.listdir(os.path.join(ROOT, "include")):                 # celes.h and celes_probe.h
+        hdr = open(os.path.join(ROOT, "include", name)).read()
+        hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+        declared |= set(re.findall(r"\b(celes_[a-z0-9_]+)\s*\(", hdr))
     assert declared == set(binding.EXPORTS)
     L = binding.lib()
     for name in declared:
@@ -185,3 +187,59 @@ def test_committed_generated_bodies_are_what_the_generators_write(gen, prefix, t
             assert new == old
     finally:
         sys.path.remove(csrc)
+
+
+@pytest.mark.parametrize("N,etile,res,levels,splits", [(1, 32, 296, 0, 0), (50, 32, 296, 0, 0), (1000, 32, 296, 0, 0),
+                                                        (10000, 32, 296, 0, 0), (100000, 32, 296, 0, 0), (10000, 24, 444, 3, 0),
+                                                        (333, 7, 5, 4, 0), (10000, 32, 296, 1, 0), (100000, 32, 296, 1, 0),
+                                                        (10000, 32, 296, 0, 6), (50, 32, 296, 0, 4), (257, 32, 296, 0, 1)])
+def test_work_partition_covers_every_pair_once(N, etile, res, levels, splits):
+    """csrc/work_partition.h through celes_plan_work: every (receiver block, emitter) is in exactly one segment, runs are
+    tile-aligned, the slots of a receiver block are contiguous and ordered by emitter, the runs of one level are equal
+    within one tile and every level is about half as long as the one before."""
+    p = celes.celes_plan_work(N, etile, res, levels, splits)
+    seg, bs = p["segments"], p["receivers_per_block"]
+    rblocks = -(-N // bs)
+    assert 1 <= bs <= 128 and rblocks * bs >= N and (rblocks - 1) * bs < N
+    assert sorted(seg[:, 4]) == list(range(len(seg)))                  # every slot written by exactly one segment
+    assert np.all(np.diff(seg[:, 0]) >= 0) and seg[:, 0].max() == p["ctas"] - 1
+    for r in range(rblocks):
+        mine = seg[seg[:, 1] == r]
+        mine = mine[np.argsort(mine[:, 2])]
+        assert len(mine) >= 1 and np.all(np.diff(mine[:, 4]) == 1)      # contiguous slots, in emitter order
+        assert mine[0, 2] == 0 and mine[-1, 3] == N
+        assert np.array_equal(mine[1:, 2], mine[:-1, 3])                # back to back, no gap, no overlap
+        assert np.all(mine[:, 2] % etile == 0) and np.all(mine[:, 3] > mine[:, 2])
+    tiles = np.zeros(p["ctas"], dtype=np.int64)
+    np.add.at(tiles, seg[:, 0], -(-(seg[:, 3] - seg[:, 2]) // etile))
+    if splits == 0:
+        lv = levels or 6
+        assert p["ctas"] <= res * lv and len(seg) <= p["ctas"] + rblocks * lv
+        assert np.all(np.diff(tiles) <= 1)                              # runs never grow along the launch order
+        if levels == 1:
+            assert p["ctas"] <= res and tiles.max() - tiles.min() <= 1  # one wave, equal work
+        if p["ctas"] > res and tiles[0] >= 64:
+            assert 0.4 <= tiles[res] / tiles[0] <= 0.6                  # second level: half the run length
+    else:
+        assert p["ctas"] == len(seg) and len(seg) <= rblocks * splits
+
+
+def test_sass_counts_of_the_built_library_match_the_committed_record():
+    """The roofline numerators bench.py reports (flops and FMA-pipe lane operations per pair) are the opcode counts of
+    the coupling kernel's per-pair loop in the BUILT libceles.so (paper_1706_02145_b200/sass_count.py, cuobjdump; no
+    GPU needed).  The committed csrc/generated/sass_counts.json must equal them, so a generator edit that changes the
+    kernel cannot leave stale constants behind; and the packed body keeps its op mix."""
+    from paper_1706_02145_b200 import sass_count
+    if sass_count.cuobjdump() is None:
+        pytest.skip("cuobjdump not installed")
+    live = sass_count.summary()
+    assert live == sass_count.committed(), "run: python -m paper_1706_02145_b200.sass_count --write"
+    for key, c in live.items():
+        f = c["fp32"]
+        assert c["flops_per_pair"] == 4 * f["FFMA2"] + 2 * (f["FMUL2"] + f["FADD2"]) + 2 * f["FFMA"] + f["FMUL"] + f["FADD"]
+        assert c["lane_ops_per_pair"] == 2 * (f["FFMA2"] + f["FMUL2"] + f["FADD2"]) + f["FFMA"] + f["FMUL"] + f["FADD"]
+    r3 = live["rotated/3"]
+    assert r3["packed_non_fma"] < 200 and r3["fp32"]["FADD2"] <= 2
+    assert r3["flops_per_pair"] / r3["lane_ops_per_pair"] > 1.75      # nearly every FMA-pipe slot is an FMA
+    b = sass_count.counts_for_bench(3)
+    assert b["flops_per_pair"] == r3["flops_per_pair"] and "live" in b["source"]

@@ -104,6 +104,22 @@ def test_radial_is_hankel_first_kind():
     assert o.radial(3, 0, x) == pytest.approx(-1j * np.exp(1j * x) / x, abs=1e-14)
 
 
+def test_radial_large_argument():
+    """Beyond x = 8000 the oracle leaves libstdc++ (which throws near 1.5e4) for the closed forms of order 0, 1 and the
+    upward recurrence: against SciPy on both sides of the switch, and continuous across it."""
+    for x in (7999.5, 8000.5, 1.2e4, 2.0e4, 5.3e4):
+        for p in range(0, 11):
+            h = o.radial(3, p, x)
+            ref = spherical_jn(p, x) + 1j * spherical_yn(p, x)
+            assert abs(h - ref) <= 2e-9 * abs(ref), (x, p)
+            assert o.radial(1, p, x).real == pytest.approx(spherical_jn(p, x), abs=2e-9 * abs(ref))
+            assert o.radial(2, p, x).real == pytest.approx(spherical_yn(p, x), abs=2e-9 * abs(ref))
+    # a block far away is what the far-field limit says: W ~ e^{ikd}/(kd) times an angular factor, |W| ~ 1/kd
+    d1, d2 = np.array([0.0, 0.0, 0.7e6]), np.array([0.0, 0.0, 1.4e6])
+    w1, w2 = o.coupling_block(2, K, d1), o.coupling_block(2, K, d2)
+    assert np.linalg.norm(w2) / np.linalg.norm(w1) == pytest.approx(0.5, rel=1e-3)
+
+
 # --------------------------------------------------------------------------- P1 addition theorem (A.5)
 @pytest.mark.parametrize("n", [(1, 1, 0), (1, 1, -1), (2, 1, 1), (1, 2, -2), (2, 2, 1), (1, 3, 3), (2, 3, -2), (2, 3, 0),
                                (1, 4, -3), (2, 4, 4)])

@@ -115,6 +115,10 @@ struct YSmem {                       // shared memory slab [q][thread] (float2):
 
 template <int LMAX>
 struct YPolicy { using type = YRegs<nmax_of(LMAX)>; };
+#ifdef CELES_SLAB3
+template <>
+struct YPolicy<3> { using type = YSmem<nmax_of(3)>; };
+#endif
 template <>
 struct YPolicy<4> { using type = YSmem<nmax_of(4)>; };
 template <>

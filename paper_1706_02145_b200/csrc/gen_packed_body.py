@@ -37,6 +37,8 @@ from rotation_tables import axial_tables, rotation_blocks  # noqa: E402
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 TOL = 1e-12
+INTERLEAVE = os.environ.get('CELES_GEN_INTERLEAVE', '0') == '1'
+_TAUVAR = re.compile(r'\b(zp|bp|bw|zw|up|uw|gp|gm|yp|zq|yw|vp|vw)(\d+_\d+)\b')
 
 
 def poly_key(cf, spow):
@@ -130,7 +132,7 @@ def count_ops(line):
     return (n["fma2"] + 2 * n["cfma2"] + n["cmul2"], n["mul2"] + n["cmul2"], n["add2"], n["fmaf"] + n["smul"])
 
 
-def emit(lmax, outdir=None, table=None):
+def emit(lmax, outdir=None, table=None, interleave=INTERLEAVE):
     H = lmax * (lmax + 2)
     P = 2 * lmax + 1
     out = []
@@ -246,8 +248,10 @@ def emit(lmax, outdir=None, table=None):
             e = f"cmul2({kk}, {x})" if e is None else f"cfma2({kk}, {x}, {e})"
         return e
 
+    tau_lines = []
     for ts in (0, 1):
         tsign = 1 if ts == 0 else -1
+        tau_start = len(out)
         w(f"    {{ // tau block {'S = (1+2)/sqrt2' if ts == 0 else 'A = (1-2)/sqrt2'}")
         # (1) load + z-rotation (real plane rotation of (u+_m, w_m)); (2) y-rotation, with g+- = u'+ -+ i w' formed
         # inside the chains: g+ seeded with -i w', g- = g+ + 2 i w'
@@ -306,6 +310,18 @@ def emit(lmax, outdir=None, table=None):
                 w(f"      yacc.put({qp}, fma2(bc2(-sm[{m}]), vw{l}_{m}, fma2(bc2(cm[{m}]), vp{l}_{m}, yacc.get({qp}))));", PHASES[7])
                 w(f"      yacc.put({qw}, fma2(bc2(cm[{m}]), vw{l}_{m}, fma2(bc2(sm[{m}]), vp{l}_{m}, yacc.get({qw}))));", PHASES[7])
         w("    }")
+        tau_lines.append(out[tau_start:])
+        del out[tau_start:]
+    if interleave:       # the two tau blocks line by line (same coefficients back to back), variables suffixed s / a
+        blk = [[_TAUVAR.sub(lambda mo, x=x: mo.group(1) + mo.group(2) + x, ln) for ln in lines[1:-1]]
+               for lines, x in zip(tau_lines, "sa")]
+        assert len(blk[0]) == len(blk[1])
+        out.append("    { // tau blocks S = (1+2)/sqrt2 and A = (1-2)/sqrt2, interleaved")
+        for ls, la in zip(*blk):
+            out.extend([ls, la])
+        out.append("    }")
+    else:
+        out.extend(tau_lines[0] + tau_lines[1])
     w("  }")
     w("};")
     outdir = outdir or os.path.join(HERE, "generated")

@@ -9,7 +9,8 @@ translations per second, N (N-1) / time, inputs resident in HBM; `e2e` is the sa
 celes_coupling_matvec_host with pinned HOST buffers (H2D + D2H inside the timed region).
 
 The path does not shard (north_star: one GPU, no collectives): --gpus N runs N independent replicas
-("replicas only"), value = pairs of all replicas / max-over-ranks time.
+("replicas only"), value = pairs of all replicas / max-over-ranks time.  --shard receivers is the
+optional receiver-sharded mode of SURVEY.md 8(e) (one all-gather of b per product, strong scaling).
 
 --impl reference times the FP64 CPU oracle (oracle/), as it stands, on a bounded sample of the same workload.
 """
@@ -40,7 +41,7 @@ FP32_LANES_PER_SM = 128
 PRECOND_EDGE_NM = 600.0     # lateral cuboid edge of the preconditioned config-5 solve in the default line
 # dram__bytes_read.sum + dram__bytes_write.sum of one coupling-kernel launch, from the ncu --set full capture
 # summarised in the named file under profiles/ (a capture, not a live measurement: ncu cannot run inside the timed run)
-NCU_DRAM_BYTES_PER_LAUNCH = {("C4", "rotated"): (131.4e6, "profiles/r01h_final_kernel_c4.md")}
+NCU_DRAM_BYTES_PER_LAUNCH = {("C4", "rotated"): (57.2e6, "profiles/r02b_kernel_c4.md")}
 
 
 def parse():
@@ -57,12 +58,18 @@ def parse():
                     help="with --solve: lateral edge (nm) of the cuboids of the block-diagonal preconditioner (0 = none)")
     ap.add_argument("--far-field", type=int, default=0, metavar="NB",
                     help="time celes_far_field on NB x 2NB directions (Gauss-Legendre x uniform azimuth) instead")
+    ap.add_argument("--near-field", type=int, default=0, metavar="NP",
+                    help="time celes_scattered_field on an NP x NP grid of points in the plane 300 nm above the slab instead")
+    ap.add_argument("--lmax", type=int, default=0, help="override the workload's truncation order (1..5)")
     ap.add_argument("--hankel", default="registers", choices=["registers", "table"],
                     help="h_p(kd) in registers (default) or from the paper's lookup table (PAPER.md:130)")
     ap.add_argument("--method", default="gmres", choices=["gmres", "bicgstab"], help="with --solve")
     ap.add_argument("--cta-trace", action="store_true",
                     help="per-CTA start / end times and SM of the coupling kernel for --levels 1 and the default partition "
                          "(needs a library built with CELES_NVCC_EXTRA=-DCELES_TRACE python -m paper_1706_02145_b200.build --force)")
+    ap.add_argument("--shard", default="none", choices=["none", "receivers"],
+                    help="with --gpus N > 1: 'receivers' shards the receiver rows over the ranks (one all-gather of b per "
+                         "product, strong scaling; SURVEY.md 8(e)) instead of running N replicas (the default, north_star)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=20.0, help="CPU work of the cpu_baseline sample")
     return ap.parse_args()
@@ -206,6 +213,28 @@ def run_reference(args, w):
         "gpu_launches": 0}))
 
 
+def precond_apply_roofline(celes, ctx, v, pc, reps: int = 20):
+    """The HBM-bound kernel of the preconditioner, z = blockdiag(M_j^{-1}) v: CUDA-event time per application and the
+    achieved bandwidth (stored blocks + the two vectors) against the measured copy bandwidth of MEASURED_PEAKS.json."""
+    import torch
+    z = torch.empty_like(v)
+    for _ in range(3):
+        celes.celes_precond_apply(ctx, v, z)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(reps):
+        celes.celes_precond_apply(ctx, v, z)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / reps
+    nbytes = pc["block_bytes"] + 2 * v.numel() * 8
+    peaks = measured_peaks()
+    peak = peaks.get("hbm_gbs", 6650.0)
+    return {"bound": "hbm", "ms": ms, "bytes": nbytes, "achieved": nbytes / ms / 1e6, "peak": peak, "unit": "GB/s",
+            "frac": nbytes / ms / 1e6 / peak, "peak_kind": "measured (MEASURED_PEAKS.json)" if "hbm_gbs" in peaks else "fallback",
+            "note": "blocks larger than L2 are re-read from HBM every application"}
+
+
 def run_solve(args, w):
     """BASELINE.json config 5: time to solution and iteration count of celes_solve; one JSON line."""
     import torch
@@ -220,7 +249,7 @@ def run_solve(args, w):
     celes.celes_solve(ctx, a_in, x, restart=30, rtol=1e-4, max_iters=3)          # warm-up (allocations, caches)
     pc = None
     if args.precond_edge > 0:
-        celes.celes_precond_setup(ctx, [args.precond_edge, args.precond_edge, 0.0])   # warm-up (cuSOLVER handle, kernels)
+        celes.celes_precond_setup(ctx, [args.precond_edge, args.precond_edge, 0.0])   # warm-up (kernel load)
     runs = []
     for _ in range(max(1, args.steps)):
         x.zero_()
@@ -234,23 +263,7 @@ def run_solve(args, w):
         runs.append((time.perf_counter() - t0, info))
     secs = [r[0] for r in runs]
     info = runs[-1][1]
-    pc_line = None
-    if pc is not None:                       # the HBM-bound kernel of the preconditioner: z = blockdiag(M_j^{-1}) v
-        z = torch.empty_like(x)
-        for _ in range(3):
-            celes.celes_precond_apply(ctx, a_in, z)
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        reps = 20
-        e0.record()
-        for _ in range(reps):
-            celes.celes_precond_apply(ctx, a_in, z)
-        e1.record()
-        torch.cuda.synchronize()
-        ms = e0.elapsed_time(e1) / reps
-        nbytes = pc["block_bytes"] + 2 * a_in.numel() * 8
-        peak = measured_peaks().get("hbm_gbs", 6650.0)
-        pc_line = {"ms": ms, "bytes": nbytes, "achieved_gbs": nbytes / ms / 1e6, "peak_gbs": peak,
-                   "frac": nbytes / ms / 1e6 / peak, "note": "blocks larger than L2 are re-read from HBM every application"}
+    pc_line = None if pc is None else precond_apply_roofline(celes, ctx, a_in, pc)
     print(json.dumps({
         "metric": "time_to_solution_s", "value": float(np.median(secs)), "unit": "s", "n_gpus": 1, "steps": len(runs),
         "warmup": 1, "higher_is_better": False, "dtype": "f32", "data": "synthetic",
@@ -298,6 +311,97 @@ def run_far_field(args, w):
         "config": {"workload": f"{w.name}: N={w.N} lmax={w.lmax}", "directions": int(al.size)},
         "roofline": {"bound": "alu", "lane_ops_per_term": lane,
                      "fma_pipe_utilisation_whole_call": lane * terms / sec / (FP32_LANES_PER_SM * sm * device_sm_clock_hz())}}))
+
+
+def run_sharded(args, w):
+    """--gpus N --shard receivers under torchrun: every rank owns a slice of the receiver rows (and of b); a step is one
+    all-gather of b (NCCL) + celes_coupling_matvec_rows on the rank's rows.  value = N (N - 1) / slowest rank's time:
+    total work is fixed, scaling = strong.  Not the default: north_star is one GPU."""
+    import torch
+    import torch.distributed as dist
+    import paper_1706_02145_b200 as celes
+    from paper_1706_02145_b200 import fields, sharding, workloads
+    world, rank = int(os.environ.get("WORLD_SIZE", "1")), int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    pos, rad = workloads.positions(w)
+    q = fields.mie_coefficients(w.lmax, w.k, rad, workloads.N_SPHERE)
+    ctx = celes.celes_setup(pos, rad, q, w.k, w.lmax, translation=args.translation)
+    slices = sharding.row_slices(w.N, world, celes.celes_work_partition(ctx)["receivers_per_block"])
+    r0, r1 = slices[rank]
+    b_rows = torch.from_numpy(workloads.gaussian_coefficients(w.N, w.nmax, w.seed_b)[r0:r1]).cuda()
+    y_rows = torch.empty_like(b_rows)
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        sharding.sharded_coupling_matvec(ctx, b_rows, slices, rank, y_rows)
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    ev = []
+    for _ in range(args.steps):
+        flush.zero_()
+        a, c = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        sharding.sharded_coupling_matvec(ctx, b_rows, slices, rank, y_rows)
+        c.record()
+        ev.append((a, c))
+    barrier()
+    clocks = sampler.stop()
+    total_ms = max_over_ranks(float(sum(a.elapsed_time(c) for a, c in ev)), world, "cuda")
+    pairs = w.N * (w.N - 1)
+    if rank == 0:
+        print(json.dumps({
+            "metric": METRIC, "value": pairs * args.steps / (total_ms * 1e-3), "unit": UNIT, "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+            "scaling": "strong", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": f"{w.name}: N={w.N} lmax={w.lmax}", "pairs_per_step": pairs,
+                       "parallelism": f"receiver rows sharded over {world} ranks, all-gather of b per product",
+                       "rows_per_rank": [e - s for s, e in slices],
+                       "l2": "flushed between timed iterations (256 MiB write)"},
+            "clocks": clocks, "gpu_launches": 3 * args.steps}))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def run_near_field(args, w):
+    """celes_scattered_field (eq. 3) on NP x NP points of a plane above the slab: time per call and
+    (point, sphere) terms per second."""
+    import torch
+    import paper_1706_02145_b200 as celes
+    from paper_1706_02145_b200 import fields, workloads
+    torch.cuda.set_device(0)
+    pos, rad = workloads.positions(w)
+    q = fields.mie_coefficients(w.lmax, w.k, rad, workloads.N_SPHERE)
+    ctx = celes.celes_setup(pos, rad, q, w.k, w.lmax)
+    b = torch.from_numpy(workloads.gaussian_coefficients(w.N, w.nmax, w.seed_b)).cuda()
+    npts = args.near_field
+    lo, hi = pos.min(axis=0), pos.max(axis=0)
+    X, Y = np.meshgrid(np.linspace(lo[0], hi[0], npts), np.linspace(lo[1], hi[1], npts), indexing="ij")
+    pts = np.stack([X.ravel(), Y.ravel(), np.full(X.size, hi[2] + rad.max() + 300.0)], axis=1)
+    for _ in range(max(2, args.warmup)):
+        celes.celes_scattered_field(ctx, b, pts)
+    times = []
+    for _ in range(max(1, args.steps)):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        celes.celes_scattered_field(ctx, b, pts)
+        e1.record()
+        torch.cuda.synchronize()
+        times.append(e0.elapsed_time(e1) * 1e-3)
+    sec = float(np.median(times))
+    terms = float(pts.shape[0]) * w.N
+    print(json.dumps({
+        "metric": "near_field_terms_per_s", "value": terms / sec, "unit": "(point,sphere)/s", "n_gpus": 1,
+        "steps": len(times), "ms_per_call": sec * 1e3, "higher_is_better": True, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"{w.name}: N={w.N} lmax={w.lmax}", "points": int(pts.shape[0])}}))
 
 
 def run_cta_trace(args, w):
@@ -400,7 +504,8 @@ def solve_c5(celes, fields, workloads, translation, precond_edge=0.0):
            "iterations": info["iterations"], "matvecs": info["matvecs"], "rel_residual": info["rel_residual"],
            "converged": bool(info["converged"])}
     if pc is not None:
-        out["preconditioner"] = dict(pc, edge_nm=precond_edge, setup_seconds=t_setup)
+        out["preconditioner"] = dict(pc, edge_nm=precond_edge, setup_seconds=t_setup,
+                                     apply_roofline=precond_apply_roofline(celes, ctx, a_in, pc))
     return out, ctx, a_in
 
 
@@ -408,6 +513,9 @@ def main():
     args = parse()
     from paper_1706_02145_b200 import workloads
     w = workloads.CONFIGS[args.workload]
+    if args.lmax:
+        import dataclasses
+        w = dataclasses.replace(w, name=f"{w.name}(lmax={args.lmax})", lmax=args.lmax)
     if args.impl == "reference":
         run_reference(args, w)
         return
@@ -416,6 +524,12 @@ def main():
         return
     if args.far_field > 0:
         run_far_field(args, w)
+        return
+    if args.near_field > 0:
+        run_near_field(args, w)
+        return
+    if args.shard == "receivers":
+        run_sharded(args, w)
         return
     if args.cta_trace:
         run_cta_trace(args, w)
@@ -513,7 +627,7 @@ def main():
             "gpu_launches": 3 * args.steps,
             "roofline": roof,
         }
-        if w.name == "C4" and world == 1:
+        if w.name == "C4" and world == 1 and not args.lmax:
             # BASELINE.json's metric names N = 1e4 as well: the same measurement on C3, reported beside the headline
             w3 = workloads.CONFIGS["C3"]
             pos3, rad3 = workloads.positions(w3)

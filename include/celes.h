@@ -42,7 +42,7 @@ typedef struct celes_ctx celes_ctx;   /* opaque; owns every device table; freed 
 
 /* Options of celes_setup (nullable -> defaults).  Zero in a field selects its default. */
 typedef struct celes_options {
-    int emitter_tile;      /* emitters staged per shared-memory tile; default 32 */
+    int emitter_tile;      /* emitters staged per shared-memory tile; default 32 (8 at lmax = 5) */
     int emitter_splits;    /* 0 (default): the (receiver block x emitter tile) grid is cut into runs of decreasing
                               length (see `levels`), one CTA each, dispatched in that order by the hardware;
                               S > 0: the emitter sum of every receiver block is cut into S equal slices, one CTA each.
@@ -168,10 +168,12 @@ int celes_solve(celes_ctx* ctx, const void* a_in_dev, void* x_dev, const celes_s
 /* Block-diagonal preconditioner (Fig. 1).  The spheres are divided into subsets G_j by an array
  * of cuboids with edge lengths edge_xyz[3] (unit U; an edge <= 0 means "do not cut along that axis") anchored at the
  * minimum corner of the centres' bounding box; for every subset the dense block M_j = (1 - T W) restricted to G_j
- * is assembled on the device, LU-factorised with partial pivoting and inverted; the context stores the inverses
- * (8 * sum_j (N_j nmax)^2 bytes).  Replaces an earlier preconditioner of the context.  Synchronises.
+ * is assembled on the device and eliminated with partial (row) pivoting through to its inverse (a blocked Gauss-Jordan
+ * elimination in the library's own kernels, all blocks side by side); the context stores the inverses
+ * (8 * sum_j (N_j nmax)^2 bytes; the set-up needs twice that while it runs).  Replaces an earlier
+ * preconditioner of the context.  Synchronises.
  * CELES_EINVAL: bad argument or a subset with more than 25600 / nmax spheres; CELES_ENOMEM: blocks do not fit;
- * CELES_ECUDA: CUDA / cuSOLVER failure or a singular block. */
+ * CELES_ECUDA: CUDA failure or a singular block. */
 int celes_precond_setup(celes_ctx* ctx, const double* edge_xyz, celes_precond_info* info, void* cuda_stream);
 
 /* z = blockdiag(M_j^{-1}) v (step 4 of PAPER.md:114).  v_dev, z_dev: device, N*nmax complex64, must not alias.

@@ -17,8 +17,7 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libceles.so")
 NVCC_FLAGS = ["-std=c++17", "-O3", *os.environ.get("CELES_NVCC_EXTRA", "").split(), "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-shared", "-Xcompiler", "-fPIC"]
-# cuSOLVER (LU of the preconditioner blocks); the CUDA toolkit's copy, found at run time through the rpath
-NVCC_LIBS = ["-lcusolver", "-Xlinker", "-rpath=/usr/local/cuda/lib64"]
+NVCC_LIBS: list[str] = []       # the CUDA runtime only
 
 
 def sources() -> list[str]:

@@ -233,7 +233,9 @@ static int setup_impl(celes_ctx** out, int N, int lmax, const double* pos_xyz, c
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, c->device) != cudaSuccess) return fail(CELES_ECUDA);
     c->sm_count = prop.multiProcessorCount;
-    c->etile = (opt && opt->emitter_tile > 0) ? opt->emitter_tile : 32;
+    // lmax = 5 spills ~0.5 KB per thread; a small tile leaves the L1 carve-out to those spills (measured: 17.8 ms with 8,
+    // 19.2 ms with 32 at N = 1e4, profiles/r02d_other_kernels.md)
+    c->etile = (opt && opt->emitter_tile > 0) ? opt->emitter_tile : (lmax >= 5 ? 8 : 32);
     c->variant = opt ? opt->translation : CELES_TRANSLATION_ROTATED;
     {   // extent of the cluster in units of 1/k: decides the range mode (celes.h: celes_options.range)
         double lo[3] = {pos_xyz[0], pos_xyz[1], pos_xyz[2]}, hi[3] = {pos_xyz[0], pos_xyz[1], pos_xyz[2]};

@@ -56,7 +56,8 @@ struct celes_ctx {
     long long* pc_blk_offset = nullptr;  // [groups]
     int* pc_cta_group = nullptr;         // [pc_ctas]
     int* pc_cta_row0 = nullptr;          // [pc_ctas]
-    float2* pc_blocks = nullptr;         // explicit inverses M_j^{-1}, column-major, back to back
+    int* pc_perm = nullptr;              // [N nmax] row permutation P_j of every block's pivoted elimination
+    float2* pc_blocks = nullptr;         // B_j = M_j^{-1} P_j^T, column-major, back to back
     float2* pc_tmp = nullptr;            // [n] work vector of the preconditioned solve
 };
 

@@ -3,10 +3,10 @@
 //   assemble_blocks_kernel  step 2: the dense blocks M_j = 1 - T W restricted to the spheres of subset G_j, from the
 //                           addition theorem (A.6)-(A.8) term by term with the run-time a5/b5 table --
 //                           an evaluation of W that is independent of the generated pair bodies
+//   (block_inverse.cuh)     step 3: pivoted elimination of every block, all blocks in the same launches
 //   block_gemv_kernel       step 4: z = blockdiag(M_j^{-1}) v.  The blocks hold the explicit inverses (obtained from
-//                           the LU factorisation of step 3), so that applying the preconditioner is one batched,
+//                           the pivoted elimination of step 3), so that applying the preconditioner is one batched,
 //                           HBM-bound matrix-vector product instead of per-block triangular solves.
-//   set_identity_kernel     helper of step 3
 #pragma once
 #include <cuda_runtime.h>
 
@@ -19,12 +19,13 @@ constexpr int kGemvRows = 128;      // rows of a block handled by one CTA of blo
 // block  M^{ab} = delta_ab 1 - T^a W^{ab}  inside the column-major n_j x n_j matrix of the subset.
 //   pair_offset [n_groups+1]: prefix sums of N_j^2;  blk_offset [n_groups]: start (in elements) of M_j in blocks;
 //   a5, b5 [H][H][P]: Re a5(l',m'|l,m|p), Im b5(l',m'|l,m|p), receiver index first (celes_translation_table layout).
+//   rounds [n_groups]: elimination rounds of the block (block_inverse.cuh); the block is written to blocks0 if even, blocks1 if odd.
 template <int LMAX>
 __global__ void __launch_bounds__(kAsmThreads) assemble_blocks_kernel(
     int n_groups, const long long* __restrict__ pair_offset, const int* __restrict__ grp_offset,
     const int* __restrict__ order, const long long* __restrict__ blk_offset, const double* __restrict__ kpos,
     const float2* __restrict__ tdiag, const float* __restrict__ a5, const float* __restrict__ b5,
-    float2* __restrict__ blocks) {
+    const int* __restrict__ rounds, float2* __restrict__ blocks0, float2* __restrict__ blocks1) {
     constexpr int H = LMAX * (LMAX + 2), NMAX = 2 * H, P = 2 * LMAX + 1;
     __shared__ float2 G[P][P];          // G[p][nu] = h_p(kd) P_p^nu(cos theta)
     __shared__ float2 E[P];             // e^{i nu phi}
@@ -40,7 +41,7 @@ __global__ void __launch_bounds__(kAsmThreads) assemble_blocks_kernel(
     const int a = local / nj, b = local - a * nj;
     const int i = order[g0 + a], ip = order[g0 + b];
     const size_t ld = (size_t)nj * NMAX;
-    float2* Mj = blocks + blk_offset[j];
+    float2* Mj = ((rounds[j] & 1) ? blocks1 : blocks0) + blk_offset[j];   // block_inverse.cuh: the last round lands in blocks0
     const int t = threadIdx.x;
     if (a == b) {                                           // W^{ii} = 0: identity block
         if (t < NMAX)
@@ -122,27 +123,21 @@ __global__ void __launch_bounds__(kAsmThreads) assemble_blocks_kernel(
         }
 }
 
-// A (column-major n x n, leading dimension n) = identity
-__global__ void set_identity_kernel(int n, float2* __restrict__ A) {
-    const size_t total = (size_t)n * n;
-    for (size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (size_t)gridDim.x * blockDim.x) {
-        const size_t c = t / n, r = t - c * n;
-        A[t] = make_float2(r == c ? 1.0f : 0.0f, 0.0f);
-    }
-}
-
 // z = blockdiag(Minv_j) v.  CTA c handles rows [row0, row0 + kGemvRows) of subset cta_group[c]; one thread per row,
 // the subset's slice of v gathered into shared memory (broadcast reads), the matrix read once, coalesced along rows.
+// The stored block is B_j = M_j^{-1} P_j^T with P_j the row permutation of the pivoted elimination (block_inverse.cuh):
+// M_j^{-1} v = B_j (P_j v), so column c of B_j meets element perm[c] of the subset's slice.
 __global__ void __launch_bounds__(kGemvRows) block_gemv_kernel(
     int nmax, const int* __restrict__ cta_group, const int* __restrict__ cta_row0, const int* __restrict__ grp_offset,
-    const int* __restrict__ order, const long long* __restrict__ blk_offset, const float2* __restrict__ blocks,
-    const float2* __restrict__ v, float2* __restrict__ z) {
+    const int* __restrict__ order, const long long* __restrict__ blk_offset, const int* __restrict__ perm,
+    const float2* __restrict__ blocks, const float2* __restrict__ v, float2* __restrict__ z) {
     extern __shared__ float2 xs[];
     const int j = cta_group[blockIdx.x], row0 = cta_row0[blockIdx.x];
     const int g0 = grp_offset[j], nj = grp_offset[j + 1] - g0, n = nj * nmax;
+    const int* pj = perm + (size_t)g0 * nmax;
     for (int c = threadIdx.x; c < n; c += kGemvRows) {
-        const int s = c / nmax;
-        xs[c] = v[(size_t)order[g0 + s] * nmax + (c - s * nmax)];
+        const int pc = pj[c], s = pc / nmax;
+        xs[c] = v[(size_t)order[g0 + s] * nmax + (pc - s * nmax)];
     }
     __syncthreads();
     const int r = row0 + threadIdx.x;

@@ -10,7 +10,7 @@
 //       first level covers half of the tiles in n_res equal runs (n_res = SMs x resident CTAs, one wave), the next a
 //       quarter, ... the last two a 2^-(levels-1) share each.  The hardware dispatches CTAs in launch order as slots
 //       free up, so the short runs at the end even out what the long ones leave uneven -- and they leave a lot: of two
-//       CTAs resident on an SM the warp scheduler favours one almost exclusively (measured: it finishes after 57 % of the
+//       CTAs resident on an SM the warp scheduler favours one almost exclusively (measured: it finishes after 58 % of the
 //       pair's time, profiles/r02_cta_trace.md), and a CTA left alone on an SM reaches only 92 % of the pipe throughput
 //       of two.  One level (a single wave of equal runs) is 5.5 % slower than many waves for that reason, six levels are
 //       within 0.2 %, with n_res * levels + rblocks partial sums instead of 56 per receiver block at N = 1e4.

@@ -312,6 +312,35 @@ def test_precond_apply_every_lmax(lmax):
     assert rel(z, orc.precond_apply(pos, w.k, w.lmax, qo, 900.0, b)) <= SOLVE_TOL
 
 
+@pytest.mark.parametrize("N", [20, 32])
+def test_block_inversion_needs_and_survives_row_interchanges(N):
+    """The pivoted elimination of the preconditioner blocks ("P_j M_j = L_j U_j"; csrc/block_inverse.cuh) on
+    a strongly coupled cluster: silicon-like spheres (n = 3.5) at filling 0.3, one cuboid, so the block is the whole
+    system and celes_precond_apply is M^{-1} v.  The FP64 LU of the same matrix interchanges hundreds of rows (asserted),
+    so the interchange, permutation-gather and multi-round paths all run.  N = 20: n = 600, panel in shared memory;
+    N = 32: n = 960, panel too large for shared memory (works in the destination buffer)."""
+    import dataclasses
+    import scipy.linalg
+    w = dataclasses.replace(workloads.scaled(workloads.C2, N), lmax=3, filling=0.3)
+    pos, rad = workloads.positions(w)
+    n_si = 3.5
+    ctx = celes.celes_setup(pos, rad, fields.mie_coefficients(w.lmax, w.k, rad, n_si), w.k, w.lmax)
+    qo = orc.mie_q(w.lmax, w.k, rad, n_si)
+    M = orc.dense_system_matrix(pos, w.k, w.lmax, qo)
+    _, piv = scipy.linalg.lu_factor(M)
+    assert int((piv != np.arange(piv.size)).sum()) > 100
+    info = celes.celes_precond_setup(ctx, 0.0)
+    assert info["n_groups"] == 1 and info["max_group_spheres"] == N
+    b = workloads.gaussian_coefficients(w.N, w.nmax, w.seed_b)
+    z = celes.celes_precond_apply(ctx, torch.from_numpy(b).cuda()).cpu().numpy()
+    ref = np.linalg.solve(M, b.astype(np.complex128).reshape(-1)).reshape(b.shape)
+    assert rel(z, ref) <= SOLVE_TOL
+    assert rel(z, orc.precond_apply(pos, w.k, w.lmax, qo, 0.0, b)) <= SOLVE_TOL
+    # and M z = b through the matrix-free system matvec (an independent evaluation of M on the device)
+    back = celes.celes_system_matvec(ctx, torch.from_numpy(z).cuda()).cpu().numpy()
+    assert rel(back, b) <= SOLVE_TOL
+
+
 def test_preconditioned_solve_same_solution_fewer_iterations():
     """Right-preconditioned GMRES: same solution as the oracle's tight solve, fewer iterations
     than the unpreconditioned solve; asking for the preconditioner before celes_precond_setup is an error."""
@@ -578,6 +607,22 @@ def test_row_slices_concatenate_to_the_full_product_bit_for_bit():
     for bad in ((-1, 10), (10, 10), (5, w.N + 1)):
         with pytest.raises(celes.CelesError):
             celes.celes_coupling_matvec_rows(ctx, bad[0], bad[1], bd)
+
+
+def test_sharded_product_of_every_rank_on_one_gpu():
+    """paper_1706_02145_b200.sharding on one GPU: the rows every rank of a 3-rank job would compute (slices aligned to
+    the receiver blocks, each from the gathered full b) concatenate to the full product bit for bit; with world = 1 the
+    sharded call IS the full product.  The all-gather itself is covered on CPU (tests/test_multi_rank.py, gloo)."""
+    from paper_1706_02145_b200 import sharding
+    w = workloads.scaled(workloads.C3, 2500)
+    pos, rad, q, ctx, b = make(w)
+    bd = torch.from_numpy(b).cuda()
+    full = celes.celes_coupling_matvec(ctx, bd).clone()
+    one = sharding.sharded_coupling_matvec(ctx, bd, [(0, w.N)], 0)
+    assert torch.equal(torch.view_as_real(one), torch.view_as_real(full))
+    slices = sharding.row_slices(w.N, 3, celes.celes_work_partition(ctx)["receivers_per_block"])
+    parts = [celes.celes_coupling_matvec_rows(ctx, r0, r1, bd).clone() for r0, r1 in slices]
+    assert torch.equal(torch.view_as_real(torch.cat(parts)), torch.view_as_real(full))
 
 
 def test_work_partitions_agree():

@@ -51,3 +51,47 @@ def test_single_rank_needs_no_process_group():
     import bench
     assert bench.max_over_ranks(12.5, 1, "cpu") == 12.5
     assert bench.job_throughput(10, 2, 1, 1000.0) == 20.0
+
+
+def test_row_slices_cover_and_balance():
+    sys.path.insert(0, ROOT)
+    from paper_1706_02145_b200 import sharding
+    for N, world, align in ((10000, 8, 127), (100000, 3, 128), (50, 4, 50), (7, 2, 1), (5, 8, 1)):
+        sl = sharding.row_slices(N, world, align)
+        assert len(sl) == world and sl[0][0] == 0 and sl[-1][1] == N
+        assert all(a[1] == b[0] for a, b in zip(sl[:-1], sl[1:])) and all(e >= s for s, e in sl)
+        assert all(s % align == 0 for s, _ in sl)
+        sizes = [e - s for s, e in sl]
+        assert max(sizes) - min(sizes) <= align
+
+
+def test_all_gather_of_row_shards_gloo_world2():
+    """The one collective of the receiver-sharded mode: every rank contributes its rows of b (unequal
+    counts) and ends up with the full vector, bit for bit, on both ranks."""
+    code = textwrap.dedent("""
+        import json, os, sys
+        import numpy as np, torch
+        import torch.distributed as dist
+        sys.path.insert(0, os.environ["PYTHONPATH"])
+        from paper_1706_02145_b200 import sharding, workloads
+        dist.init_process_group("gloo")
+        rank, world = dist.get_rank(), dist.get_world_size()
+        N, nmax = 301, 30
+        b = torch.from_numpy(workloads.gaussian_coefficients(N, nmax, 77))
+        ok = True
+        for align in (1, 128):
+            slices = sharding.row_slices(N, world, align)
+            r0, r1 = slices[rank]
+            full = sharding.all_gather_rows(b[r0:r1].clone(), slices, rank)
+            ok = ok and full.shape == b.shape and bool(torch.equal(torch.view_as_real(full), torch.view_as_real(b)))
+        flags = [None] * world
+        dist.all_gather_object(flags, ok)
+        if rank == 0:
+            print("RESULT " + json.dumps({"world": world, "ok": flags, "slices": sharding.row_slices(N, world, 128)}))
+        dist.destroy_process_group()
+    """)
+    r = _torchrun(code, port=29613)
+    assert r.returncode == 0, r.stderr[-2000:]
+    out = json.loads([l for l in r.stdout.splitlines() if l.startswith("RESULT ")][0][7:])
+    assert out["world"] == 2 and out["ok"] == [True, True]
+    assert out["slices"] == [[0, 128], [128, 301]]

@@ -6,7 +6,8 @@
 // each of the spheres, adding up the contribution of all spheres"; I_j = 2 pi^2/(omega k mu_0) |g_j|^2.
 //
 //   far_field_coefficients_kernel  c[d][j][n] = B_nj(beta_d) exp(i m alpha_d) / (2 pi), B from (A.14), PAPER.md:280 (FP64)
-//   far_field_kernel        device: one thread per (direction, polarisation); the spheres' coefficients and k r_i are
+//   far_field_kernel        device: one thread per direction (both polarisations; lmax <= 3) or per (direction,
+//                           polarisation); the spheres' coefficients and k r_i are
 //                           staged through shared memory in tiles (all lanes read the same sphere: broadcasts); the
 //                           phase k.r_i is formed and reduced mod 2 pi in FP64 (it reaches ~1e3 rad), the rest is packed
 //                           FP32 (the c_n of the thread live in registers).  O(N n_dir nmax), bound by the FMA pipe.
@@ -96,9 +97,12 @@ __global__ void far_field_coefficients_kernel(int lmax, int n_dir, const double*
     }
 }
 
-// grid = (ceil(n_rows / kFarThreads), splits): CTA (x, y) sums the spheres [y * chunk, (y+1) * chunk) for its rows and
-// writes gpart[y][row]; far_field_reduce_kernel adds the splits in a fixed order.
-template <int NMAX>
+// grid = (ceil(n_rows / (POLS kFarThreads)), splits): CTA (x, y) sums the spheres [y * chunk, (y+1) * chunk) for its rows
+// and writes gpart[y][row]; far_field_reduce_kernel adds the splits in a fixed order.  A thread owns POLS consecutive rows:
+// POLS = 1, one (direction, polarisation); POLS = 2 (n_rows even), both polarisations of one direction, which share the
+// FP64 phase, the sine / cosine and every shared-memory load of b (the LDS broadcast path is what limits POLS = 1:
+// profiles/r02d_other_kernels.md) at twice the coefficient registers -- used while 2 NMAX complex coefficients fit.
+template <int NMAX, int POLS>
 __global__ void __launch_bounds__(kFarThreads) far_field_kernel(int N, int chunk, int n_rows,
                                                                 const double* __restrict__ kpos,
                                                                 const float2* __restrict__ b,
@@ -106,15 +110,19 @@ __global__ void __launch_bounds__(kFarThreads) far_field_kernel(int N, int chunk
                                                                 const double* __restrict__ dir, float2* __restrict__ gpart) {
     __shared__ __align__(16) float2 sb[kFarTile * NMAX];
     __shared__ double spos[kFarTile * 3];
-    const int row = blockIdx.x * kFarThreads + threadIdx.x;          // row = direction * 2 + (j - 1)
+    const int row = (blockIdx.x * kFarThreads + threadIdx.x) * POLS;   // row = direction * 2 + (j - 1)
     const bool active = row < n_rows;
-    const int rc = active ? row : n_rows - 1;
-    float2 c[NMAX];
+    const int rc = active ? row : n_rows - POLS;
+    float2 c[POLS][NMAX];
 #pragma unroll
-    for (int n = 0; n < NMAX; ++n) c[n] = coef[(size_t)rc * NMAX + n];
+    for (int p = 0; p < POLS; ++p)
+#pragma unroll
+        for (int n = 0; n < NMAX; ++n) c[p][n] = coef[(size_t)(rc + p) * NMAX + n];
     const int d = rc >> 1;
     const double nx = dir[3 * d], ny = dir[3 * d + 1], nz = dir[3 * d + 2];
-    float2 acc = make_float2(0.f, 0.f);
+    float2 acc[POLS];
+#pragma unroll
+    for (int p = 0; p < POLS; ++p) acc[p] = make_float2(0.f, 0.f);
     const int s_begin = blockIdx.y * chunk, s_end = min(N, s_begin + chunk);
     for (int t0 = s_begin; t0 < s_end; t0 += kFarTile) {
         const int ne = min(kFarTile, s_end - t0);
@@ -133,24 +141,34 @@ __global__ void __launch_bounds__(kFarThreads) far_field_kernel(int N, int chunk
             float sn, cs;
             __sincosf((float)ph, &sn, &cs);                         // |ph| <= pi after the FP64 reduction: hardware path
             const float4* be = reinterpret_cast<const float4*>(sb + e * NMAX);
-            // sum_n c_n b_n = P + i Q, two independent chains each
-            float2 P0 = make_float2(0.f, 0.f), Q0 = P0, P1 = P0, Q1 = P0;
+            // sum_n c_n b_n = P + i Q per polarisation, two independent chains each
+            float2 P0[POLS], Q0[POLS], P1[POLS], Q1[POLS];
+#pragma unroll
+            for (int p = 0; p < POLS; ++p) P0[p] = Q0[p] = P1[p] = Q1[p] = make_float2(0.f, 0.f);
 #pragma unroll
             for (int n = 0; n < NMAX; n += 2) {
                 const float4 bb = be[n >> 1];
                 const float2 b0 = make_float2(bb.x, bb.y), b1 = make_float2(bb.z, bb.w);
-                P0 = fma2(bc2(c[n].x), b0, P0);
-                Q0 = fma2(bc2(c[n].y), b0, Q0);
-                P1 = fma2(bc2(c[n + 1].x), b1, P1);
-                Q1 = fma2(bc2(c[n + 1].y), b1, Q1);
+#pragma unroll
+                for (int p = 0; p < POLS; ++p) {
+                    P0[p] = fma2(bc2(c[p][n].x), b0, P0[p]);
+                    Q0[p] = fma2(bc2(c[p][n].y), b0, Q0[p]);
+                    P1[p] = fma2(bc2(c[p][n + 1].x), b1, P1[p]);
+                    Q1[p] = fma2(bc2(c[p][n + 1].y), b1, Q1[p]);
+                }
             }
-            const float2 P = add2(P0, P1), Q = add2(Q0, Q1);
-            const float2 s = add2(P, make_float2(-Q.y, Q.x));
-            acc = fma2(bc2(cs), s, acc);
-            acc = fma2(bc2(sn), make_float2(-s.y, s.x), acc);
+#pragma unroll
+            for (int p = 0; p < POLS; ++p) {
+                const float2 P = add2(P0[p], P1[p]), Q = add2(Q0[p], Q1[p]);
+                const float2 s = add2(P, make_float2(-Q.y, Q.x));
+                acc[p] = fma2(bc2(cs), s, acc[p]);
+                acc[p] = fma2(bc2(sn), make_float2(-s.y, s.x), acc[p]);
+            }
         }
     }
-    if (active) gpart[(size_t)blockIdx.y * n_rows + row] = acc;
+    if (active)
+#pragma unroll
+        for (int p = 0; p < POLS; ++p) gpart[(size_t)blockIdx.y * n_rows + row + p] = acc[p];
 }
 
 __global__ void far_field_reduce_kernel(int n_rows, int splits, const float2* __restrict__ gpart, float2* __restrict__ g) {

@@ -47,7 +47,9 @@ int celes_far_field(celes_ctx* ctx, const void* b_dev, int n_dir, const double* 
     for (int d = 0; d < n_dir; ++d)
         if (!std::isfinite(alpha[d]) || !std::isfinite(beta[d])) return CELES_EINVAL;
     cudaStream_t s = (cudaStream_t)cuda_stream;
-    const int nmax = ctx->nmax, rows = 2 * n_dir, gx = (rows + celes::kFarThreads - 1) / celes::kFarThreads;
+    // a thread owns both polarisations of a direction while 2 nmax complex coefficients fit in registers (lmax <= 3)
+    const int pols = ctx->lmax <= 3 ? 2 : 1;
+    const int nmax = ctx->nmax, rows = 2 * n_dir, gx = (rows / pols + celes::kFarThreads - 1) / celes::kFarThreads;
     // split the sphere sum so that the grid has about four CTAs per SM-slot pair, at least 4 tiles per CTA
     int splits = std::max(1, std::min((8 * ctx->sm_count + gx - 1) / gx, std::max(1, ctx->N / (4 * celes::kFarTile))));
     const int chunk = ((ctx->N + splits - 1) / splits + celes::kFarTile - 1) / celes::kFarTile * celes::kFarTile;
@@ -67,11 +69,11 @@ int celes_far_field(celes_ctx* ctx, const void* b_dev, int n_dir, const double* 
         const float2* b = (const float2*)b_dev;
         dim3 grid(gx, splits);
         switch (ctx->lmax) {
-            case 1: celes::far_field_kernel<6><<<grid, celes::kFarThreads, 0, s>>>(ctx->N, chunk, rows, ctx->kpos, b, d_coef, d_dir, d_part); break;
-            case 2: celes::far_field_kernel<16><<<grid, celes::kFarThreads, 0, s>>>(ctx->N, chunk, rows, ctx->kpos, b, d_coef, d_dir, d_part); break;
-            case 3: celes::far_field_kernel<30><<<grid, celes::kFarThreads, 0, s>>>(ctx->N, chunk, rows, ctx->kpos, b, d_coef, d_dir, d_part); break;
-            case 4: celes::far_field_kernel<48><<<grid, celes::kFarThreads, 0, s>>>(ctx->N, chunk, rows, ctx->kpos, b, d_coef, d_dir, d_part); break;
-            case 5: celes::far_field_kernel<70><<<grid, celes::kFarThreads, 0, s>>>(ctx->N, chunk, rows, ctx->kpos, b, d_coef, d_dir, d_part); break;
+            case 1: celes::far_field_kernel<6, 2><<<grid, celes::kFarThreads, 0, s>>>(ctx->N, chunk, rows, ctx->kpos, b, d_coef, d_dir, d_part); break;
+            case 2: celes::far_field_kernel<16, 2><<<grid, celes::kFarThreads, 0, s>>>(ctx->N, chunk, rows, ctx->kpos, b, d_coef, d_dir, d_part); break;
+            case 3: celes::far_field_kernel<30, 2><<<grid, celes::kFarThreads, 0, s>>>(ctx->N, chunk, rows, ctx->kpos, b, d_coef, d_dir, d_part); break;
+            case 4: celes::far_field_kernel<48, 1><<<grid, celes::kFarThreads, 0, s>>>(ctx->N, chunk, rows, ctx->kpos, b, d_coef, d_dir, d_part); break;
+            case 5: celes::far_field_kernel<70, 1><<<grid, celes::kFarThreads, 0, s>>>(ctx->N, chunk, rows, ctx->kpos, b, d_coef, d_dir, d_part); break;
             default: rc = CELES_EINVAL;
         }
         if (!rc) celes::far_field_reduce_kernel<<<(rows + 255) / 256, 256, 0, s>>>(rows, splits, d_part, (float2*)g_dev);

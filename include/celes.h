@@ -170,8 +170,8 @@ int celes_solve(celes_ctx* ctx, const void* a_in_dev, void* x_dev, const celes_s
  * minimum corner of the centres' bounding box; for every subset the dense block M_j = (1 - T W) restricted to G_j
  * is assembled on the device and eliminated with partial (row) pivoting through to its inverse (a blocked Gauss-Jordan
  * elimination in the library's own kernels, all blocks side by side); the context stores the inverses
- * (8 * sum_j (N_j nmax)^2 bytes; the set-up needs twice that while it runs).  Replaces an earlier
- * preconditioner of the context.  Synchronises.
+ * (8 * sum_j (N_j nmax)^2 bytes; the elimination runs in place).  Replaces an earlier preconditioner of
+ * the context, reusing its block buffer if the new blocks fit.  Synchronises.
  * CELES_EINVAL: bad argument or a subset with more than 25600 / nmax spheres; CELES_ENOMEM: blocks do not fit;
  * CELES_ECUDA: CUDA failure or a singular block. */
 int celes_precond_setup(celes_ctx* ctx, const double* edge_xyz, celes_precond_info* info, void* cuda_stream);

@@ -12,9 +12,11 @@
 //   gj_update_kernel  strips of 64 columns, walked in 64 x 64 tiles, of all other columns:  new[i][j] = (i in [c0,c1) ? 0 : old[src[i]][j])
 //                     + sum_t G[i][c0+t] old[src[c0+t]][j]  -- a rank-32 complex update in packed FFMA2.
 //
-// The two buffers alternate (no tile reads what another tile of the same launch writes); a block with R rounds is
-// assembled into buffer R mod 2, so that every block's last round lands in buffer 0, the one that is kept.  After the
-// last round buffer 0 holds B = (P A)^{-1} = A^{-1} P^T with P the accumulated row permutation `net` (row i of P A is row
+// Everything happens IN PLACE in the one buffer that is kept.  The panel kernel owns the panel's columns; an update CTA
+// owns ALL rows of its 64 columns and walks them top to bottom, so a tile only ever needs (a) its own rows, not yet
+// overwritten, (b) the pivot rows and (c) the rows an interchange moved below the panel -- at most 32 per round, listed by
+// the panel kernel (`disp_rows`) -- and it gathers (b) and (c) into shared memory before it writes anything.  After the
+// last round the buffer holds B = (P A)^{-1} = A^{-1} P^T with P the accumulated row permutation `net` (row i of P A is row
 // net[i] of A): z = A^{-1} v = B (P v), i.e. block_gemv_kernel reads v through net (precond_kernels.cuh).
 #pragma once
 #include <cuda_runtime.h>
@@ -32,9 +34,10 @@ struct GjBlocks {                  // device tables of the blocks, shared by bot
     const int* by_size;            // [G] block indices, largest first (the active blocks of a round are a prefix)
     const int* grp_offset;         // [G+1] sphere offsets: n_j = (grp_offset[j+1] - grp_offset[j]) nmax; row tables start at grp_offset[j] nmax
     const long long* blk_offset;   // [G] element offset of block j in either buffer
-    const int* rounds;             // [G] ceil(n_j / kGjNb)
-    float2 *buf0, *buf1;
+    float2* buf;                   // the blocks, column-major, back to back
     int* src_row;                  // [N nmax] row interchange table of the current round
+    int* disp_count;               // [G] rows below the panel whose content an interchange replaced (<= kGjNb)
+    int* disp_rows;                // [G][kGjNb] their positions
     int* net;                      // [N nmax] accumulated permutation
     int* info;                     // [G] 1 = singular (zero or non-finite pivot)
 };
@@ -53,15 +56,15 @@ __global__ void __launch_bounds__(kGjThreads) gj_panel_kernel(GjBlocks B, int ro
     const int c0 = round * kGjNb;
     if (c0 >= n) return;
     const int w = min(kGjNb, n - c0);
-    const int R = B.rounds[j];
-    const float2* old = (((R - round) & 1) ? B.buf1 : B.buf0) + B.blk_offset[j];
-    float2* neu = (((R - round - 1) & 1) ? B.buf1 : B.buf0) + B.blk_offset[j];
+    float2* neu = B.buf + B.blk_offset[j];
     int* src = reinterpret_cast<int*>(gj_smem);
     const bool in_smem = (long long)n * w <= panel_capacity;
     float2* P = in_smem ? reinterpret_cast<float2*>(gj_smem + (size_t)src_capacity * sizeof(int)) : neu + (size_t)c0 * n;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    for (int e = tid; e < n * w; e += kGjThreads) P[e] = old[(size_t)c0 * n + e];      // column-major panel, leading dimension n
+    if (in_smem)
+        for (int e = tid; e < n * w; e += kGjThreads) P[e] = neu[(size_t)c0 * n + e];  // column-major panel, leading dimension n
     for (int i = tid; i < n; i += kGjThreads) src[i] = i;
+    if (tid == 0) B.disp_count[j] = 0;
     __syncthreads();
     for (int s = 0; s < w; ++s) {
         const int pr = c0 + s;
@@ -127,6 +130,7 @@ __global__ void __launch_bounds__(kGjThreads) gj_panel_kernel(GjBlocks B, int ro
     for (int i = tid; i < n; i += kGjThreads) {
         const int si = src[i];
         B.src_row[rowbase + i] = si;
+        if (i >= c0 + w && si != i) B.disp_rows[(size_t)j * kGjNb + atomicAdd(&B.disp_count[j], 1)] = i;   // order is immaterial
         src[i] = round == 0 ? si : B.net[rowbase + si];                    // net_new[i] = net_old[src[i]]
     }
     __syncthreads();
@@ -134,11 +138,13 @@ __global__ void __launch_bounds__(kGjThreads) gj_panel_kernel(GjBlocks B, int ro
 }
 
 // strip_off [n_active + 1]: prefix sums of ceil(n_j / 64) over the blocks in by_size order.  One CTA per strip of 64
-// columns: the pivot rows of the strip are gathered once, then the CTA walks down the strip in 64 x 64 tiles, loading the
-// next tile (old values + the panel's rows) into registers while the current one is being multiplied.
+// columns: the pivot rows and the displaced rows of the strip are gathered once, BEFORE anything is written, then the CTA
+// walks down the strip in 64 x 64 tiles in place, loading the next tile (old values of its own rows + the panel's rows)
+// into registers while the current one is being multiplied.
 __global__ void __launch_bounds__(256, 2) gj_update_kernel(GjBlocks B, int round, int n_active, const long long* __restrict__ strip_off) {
     __shared__ __align__(16) float2 As[kGjNb][kGjTile];      // G[i0 + row][c0 + t]
     __shared__ __align__(16) float2 Bs[kGjNb][kGjTile];      // old[src[c0 + t]][j0 + col]
+    __shared__ float2 Ds[kGjNb][kGjTile];                    // old[src[disp[k]]][j0 + col]: rows an interchange moved below the panel                    // (3 x 16 KB: the static shared-memory limit)
     int lo = 0, hi = n_active;
     const long long bid = blockIdx.x;
     while (hi - lo > 1) {
@@ -154,17 +160,20 @@ __global__ void __launch_bounds__(256, 2) gj_update_kernel(GjBlocks B, int round
     const int j0 = (int)(bid - strip_off[lo]) * kGjTile;
     const int jend = min(n, j0 + kGjTile);
     if (j0 >= c0 && jend <= c1) return;                                    // every column of the strip is a panel column
-    const int R = B.rounds[j];
-    const float2* old = (((R - round) & 1) ? B.buf1 : B.buf0) + B.blk_offset[j];
-    float2* neu = (((R - round - 1) & 1) ? B.buf1 : B.buf0) + B.blk_offset[j];
+    float2* neu = B.buf + B.blk_offset[j];
+    const float2* old = neu;                                               // in place: see the header of this file
     const int* src = B.src_row + (size_t)g0 * B.nmax;
+    const int ndisp = B.disp_count[j];
+    const int* disp = B.disp_rows + (size_t)j * kGjNb;
     const int tid = threadIdx.x;
     const int tx = tid & 15, ty = tid >> 4;
     const float2 zero = make_float2(0.f, 0.f);
     for (int e = tid; e < kGjNb * kGjTile; e += 256) {
         const int t = e >> 6, col = j0 + (e & 63);
         Bs[t][e & 63] = (t < w && col < n) ? old[(size_t)col * n + src[c0 + t]] : zero;
+        if (t < ndisp && col < n) Ds[t][e & 63] = old[(size_t)col * n + src[disp[t]]];
     }
+    __syncthreads();                                                       // everything gathered before the first store
     float2 pa[8], pc[4][4];
     auto prefetch = [&](int tm) {
         const int i0 = tm * kGjTile;
@@ -177,13 +186,18 @@ __global__ void __launch_bounds__(256, 2) gj_update_kernel(GjBlocks B, int round
 #pragma unroll
         for (int a = 0; a < 4; ++a) {
             const int row = i0 + tx + 16 * a;                              // lanes walk down a column: coalesced
-            srow[a] = row >= n ? -1 : (row < c0 ? row : (row < c1 ? -1 : src[row]));
+            // >= 0: the row itself (not yet overwritten: tiles are walked top to bottom); -1: zero (pivot row or outside);
+            // <= -2: displaced row, slot -2 - srow of Ds
+            srow[a] = (row >= n || (row >= c0 && row < c1)) ? -1 : row;
+            if (row >= c1 && row < n && ndisp > 0 && src[row] != row)
+                for (int k = 0; k < ndisp; ++k) if (disp[k] == row) srow[a] = -2 - k;
         }
 #pragma unroll
         for (int b = 0; b < 4; ++b) {
-            const int col = j0 + 4 * ty + b;
+            const int col = j0 + 4 * ty + b, cl = 4 * ty + b;
 #pragma unroll
-            for (int a = 0; a < 4; ++a) pc[a][b] = (col < n && srow[a] >= 0) ? old[(size_t)col * n + srow[a]] : zero;
+            for (int a = 0; a < 4; ++a)
+                pc[a][b] = col >= n ? zero : (srow[a] >= 0 ? old[(size_t)col * n + srow[a]] : (srow[a] == -1 ? zero : Ds[-2 - srow[a]][cl]));
         }
     };
     prefetch(0);

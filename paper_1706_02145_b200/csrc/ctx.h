@@ -51,6 +51,7 @@ struct celes_ctx {
     bool pc_ready = false;
     int pc_groups = 0, pc_max_n = 0, pc_ctas = 0;
     long long pc_elems = 0;      // sum_j n_j^2
+    long long pc_capacity = 0;   // elements allocated behind pc_blocks (a later set-up that fits reuses the buffer)
     int* pc_order = nullptr;     // [N]
     int* pc_grp_offset = nullptr;        // [groups+1]
     long long* pc_blk_offset = nullptr;  // [groups]

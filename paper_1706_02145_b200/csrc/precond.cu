@@ -21,7 +21,7 @@ void celes::host::free_precond(celes_ctx* c) {
     cudaFree(c->pc_cta_row0); cudaFree(c->pc_perm); cudaFree(c->pc_blocks); cudaFree(c->pc_tmp);
     c->pc_order = c->pc_grp_offset = c->pc_cta_group = c->pc_cta_row0 = c->pc_perm = nullptr;
     c->pc_blk_offset = nullptr; c->pc_blocks = c->pc_tmp = nullptr;
-    c->pc_ready = false; c->pc_groups = c->pc_max_n = c->pc_ctas = 0; c->pc_elems = 0;
+    c->pc_ready = false; c->pc_groups = c->pc_max_n = c->pc_ctas = 0; c->pc_elems = 0; c->pc_capacity = 0;
 }
 
 // z = blockdiag(M_j^{-1}) v  (step 4)
@@ -67,7 +67,12 @@ int celes_partition(int N, const double* pos_xyz, const double* edge_xyz, int* g
 // batched matrix-vector product (block_gemv_kernel).
 static int precond_setup_impl(celes_ctx* ctx, const double* edge_xyz, celes_precond_info* info, cudaStream_t s) {
     const auto t_start = std::chrono::steady_clock::now();
+    // a set-up that replaces an earlier one keeps the block buffer if the new blocks fit (no GB-sized free + allocation)
+    float2* kept = ctx->pc_blocks;
+    const long long kept_capacity = ctx->pc_capacity;
+    ctx->pc_blocks = nullptr;
     free_precond(ctx);
+    ctx->pc_blocks = kept; ctx->pc_capacity = kept_capacity;         // owned by the context again: every exit path frees or keeps it
     celes::Partition part;
     if (!celes::build_partition(ctx->N, ctx->pos.data(), edge_xyz, part)) return CELES_EINVAL;
     const int G = part.n_groups(), nmax = ctx->nmax;
@@ -101,11 +106,10 @@ static int precond_setup_impl(celes_ctx* ctx, const double* edge_xyz, celes_prec
 
     long long *d_pair_off = nullptr, *d_tile_off = nullptr;
     float *d_a5 = nullptr, *d_b5 = nullptr;
-    int *d_info = nullptr, *d_rounds = nullptr, *d_by_size = nullptr, *d_src_row = nullptr;
-    float2* d_buf1 = nullptr;
+    int *d_info = nullptr, *d_by_size = nullptr, *d_src_row = nullptr, *d_disp_count = nullptr, *d_disp_rows = nullptr;
     auto cleanup = [&](int code) {
-        cudaFree(d_pair_off); cudaFree(d_tile_off); cudaFree(d_a5); cudaFree(d_b5); cudaFree(d_info); cudaFree(d_rounds);
-        cudaFree(d_by_size); cudaFree(d_src_row); cudaFree(d_buf1);
+        cudaFree(d_pair_off); cudaFree(d_tile_off); cudaFree(d_a5); cudaFree(d_b5); cudaFree(d_info);
+        cudaFree(d_by_size); cudaFree(d_src_row); cudaFree(d_disp_count); cudaFree(d_disp_rows);
         if (code != CELES_OK) free_precond(ctx);
         return code;
     };
@@ -124,16 +128,21 @@ static int precond_setup_impl(celes_ctx* ctx, const double* edge_xyz, celes_prec
     PC_TRY(cudaMalloc(&ctx->pc_cta_group, sizeof(int) * cta_group.size()));
     PC_TRY(cudaMalloc(&ctx->pc_cta_row0, sizeof(int) * cta_row0.size()));
     PC_TRY(cudaMalloc(&ctx->pc_perm, sizeof(int) * rows));
-    PC_TRY(cudaMalloc(&ctx->pc_blocks, sizeof(float2) * (size_t)elems));
+    if (ctx->pc_capacity < elems) {
+        cudaFree(ctx->pc_blocks);
+        ctx->pc_blocks = nullptr; ctx->pc_capacity = 0;
+        PC_TRY(cudaMalloc(&ctx->pc_blocks, sizeof(float2) * (size_t)elems));
+        ctx->pc_capacity = elems;
+    }
     PC_TRY(cudaMalloc(&ctx->pc_tmp, sizeof(float2) * rows));
-    PC_TRY(cudaMalloc(&d_buf1, sizeof(float2) * (size_t)elems));                 // second buffer of the elimination, released below
     PC_TRY(cudaMalloc(&d_src_row, sizeof(int) * rows));
     PC_TRY(cudaMalloc(&d_pair_off, sizeof(long long) * (G + 1)));
     PC_TRY(cudaMalloc(&d_tile_off, sizeof(long long) * (G + 1)));
     PC_TRY(cudaMalloc(&d_a5, sizeof(float) * a5f.size()));
     PC_TRY(cudaMalloc(&d_b5, sizeof(float) * b5f.size()));
     PC_TRY(cudaMalloc(&d_info, sizeof(int) * (size_t)G));
-    PC_TRY(cudaMalloc(&d_rounds, sizeof(int) * (size_t)G));
+    PC_TRY(cudaMalloc(&d_disp_count, sizeof(int) * (size_t)G));
+    PC_TRY(cudaMalloc(&d_disp_rows, sizeof(int) * (size_t)G * celes::kGjNb));
     PC_TRY(cudaMalloc(&d_by_size, sizeof(int) * (size_t)G));
     PC_TRY(cudaMemcpyAsync(ctx->pc_order, part.order.data(), sizeof(int) * ctx->N, cudaMemcpyHostToDevice, s));
     PC_TRY(cudaMemcpyAsync(ctx->pc_grp_offset, part.offset.data(), sizeof(int) * (G + 1), cudaMemcpyHostToDevice, s));
@@ -144,15 +153,14 @@ static int precond_setup_impl(celes_ctx* ctx, const double* edge_xyz, celes_prec
     PC_TRY(cudaMemcpyAsync(d_tile_off, tile_off.data(), sizeof(long long) * (G + 1), cudaMemcpyHostToDevice, s));
     PC_TRY(cudaMemcpyAsync(d_a5, a5f.data(), sizeof(float) * a5f.size(), cudaMemcpyHostToDevice, s));
     PC_TRY(cudaMemcpyAsync(d_b5, b5f.data(), sizeof(float) * b5f.size(), cudaMemcpyHostToDevice, s));
-    PC_TRY(cudaMemcpyAsync(d_rounds, rounds.data(), sizeof(int) * (size_t)G, cudaMemcpyHostToDevice, s));
     PC_TRY(cudaMemcpyAsync(d_by_size, by_size.data(), sizeof(int) * (size_t)G, cudaMemcpyHostToDevice, s));
     PC_TRY(cudaMemsetAsync(d_info, 0, sizeof(int) * (size_t)G, s));
-    // (2) assemble every block (into the buffer from which its last elimination round lands in pc_blocks)
+    // (2) assemble every block
     {
         const unsigned grid = (unsigned)pair_off[G];
 #define PC_ASM(L)                                                                                              \
     celes::assemble_blocks_kernel<L><<<grid, celes::kAsmThreads, 0, s>>>(G, d_pair_off, ctx->pc_grp_offset,     \
-        ctx->pc_order, ctx->pc_blk_offset, ctx->kpos, ctx->tdiag, d_a5, d_b5, d_rounds, ctx->pc_blocks, d_buf1)
+        ctx->pc_order, ctx->pc_blk_offset, ctx->kpos, ctx->tdiag, d_a5, d_b5, ctx->pc_blocks)
         switch (ctx->lmax) {
             case 1: PC_ASM(1); break;
             case 2: PC_ASM(2); break;
@@ -174,8 +182,8 @@ static int precond_setup_impl(celes_ctx* ctx, const double* edge_xyz, celes_prec
         const long long room = ((long long)optin - (long long)src_capacity * (long long)sizeof(int)) / (long long)sizeof(float2);
         const long long panel_capacity = std::max(0LL, std::min(room, max_n * celes::kGjNb));   // elements; larger panels work in global memory
         const size_t smem = (size_t)src_capacity * sizeof(int) + (size_t)panel_capacity * sizeof(float2);
-        celes::GjBlocks B{nmax, d_by_size, ctx->pc_grp_offset, ctx->pc_blk_offset, d_rounds, ctx->pc_blocks, d_buf1,
-                          d_src_row, ctx->pc_perm, d_info};
+        celes::GjBlocks B{nmax, d_by_size, ctx->pc_grp_offset, ctx->pc_blk_offset, ctx->pc_blocks, d_src_row, d_disp_count,
+                          d_disp_rows, ctx->pc_perm, d_info};
         const int max_rounds = rounds[by_size[0]];
         int n_active = G;
         for (int r = 0; r < max_rounds; ++r) {

@@ -19,16 +19,16 @@ constexpr int kGemvRows = 128;      // rows of a block handled by one CTA of blo
 // block  M^{ab} = delta_ab 1 - T^a W^{ab}  inside the column-major n_j x n_j matrix of the subset.
 //   pair_offset [n_groups+1]: prefix sums of N_j^2;  blk_offset [n_groups]: start (in elements) of M_j in blocks;
 //   a5, b5 [H][H][P]: Re a5(l',m'|l,m|p), Im b5(l',m'|l,m|p), receiver index first (celes_translation_table layout).
-//   rounds [n_groups]: elimination rounds of the block (block_inverse.cuh); the block is written to blocks0 if even, blocks1 if odd.
 template <int LMAX>
 __global__ void __launch_bounds__(kAsmThreads) assemble_blocks_kernel(
     int n_groups, const long long* __restrict__ pair_offset, const int* __restrict__ grp_offset,
     const int* __restrict__ order, const long long* __restrict__ blk_offset, const double* __restrict__ kpos,
     const float2* __restrict__ tdiag, const float* __restrict__ a5, const float* __restrict__ b5,
-    const int* __restrict__ rounds, float2* __restrict__ blocks0, float2* __restrict__ blocks1) {
+    float2* __restrict__ blocks) {
     constexpr int H = LMAX * (LMAX + 2), NMAX = 2 * H, P = 2 * LMAX + 1;
     __shared__ float2 G[P][P];          // G[p][nu] = h_p(kd) P_p^nu(cos theta)
     __shared__ float2 E[P];             // e^{i nu phi}
+    __shared__ float2 tile[NMAX][NMAX + 1];   // tile[n'][n]: the block, staged so that it leaves in runs of consecutive rows
     // subset of this pair: binary search in the prefix sums
     const long long bid = blockIdx.x;
     int lo = 0, hi = n_groups;
@@ -41,12 +41,14 @@ __global__ void __launch_bounds__(kAsmThreads) assemble_blocks_kernel(
     const int a = local / nj, b = local - a * nj;
     const int i = order[g0 + a], ip = order[g0 + b];
     const size_t ld = (size_t)nj * NMAX;
-    float2* Mj = ((rounds[j] & 1) ? blocks1 : blocks0) + blk_offset[j];   // block_inverse.cuh: the last round lands in blocks0
+    float2* Mj = blocks + blk_offset[j];
     const int t = threadIdx.x;
+    float2* out = Mj + (size_t)(a * NMAX) + (size_t)(b * NMAX) * ld;   // element (n, n') at out[n + n' ld]
     if (a == b) {                                           // W^{ii} = 0: identity block
-        if (t < NMAX)
-            for (int n = 0; n < NMAX; ++n)
-                Mj[(size_t)(a * NMAX + n) + (size_t)(b * NMAX + t) * ld] = make_float2(n == t ? 1.0f : 0.0f, 0.0f);
+        for (int e = t; e < NMAX * NMAX; e += kAsmThreads) {
+            const int c = e / NMAX, n = e - c * NMAX;
+            out[(size_t)c * ld + n] = make_float2(n == c ? 1.0f : 0.0f, 0.0f);
+        }
         return;
     }
     // geometry of d = r_i - r_i'; subtraction in FP64 as in the coupling kernel
@@ -91,12 +93,12 @@ __global__ void __launch_bounds__(kAsmThreads) assemble_blocks_kernel(
         E[nu] = make_float2(cr, ci);
     }
     __syncthreads();
-    if (t >= NMAX) return;
+    if (t < NMAX) {
     const int taup = t / H, cq = t - taup * H;              // emitter n' = (tau', l', m')
     int lp = 1;
     while ((lp + 1) * (lp + 1) - 1 <= cq) ++lp;
     const int mp = cq - (lp * lp - 1) - lp;
-    float2* col = Mj + (size_t)(a * NMAX) + (size_t)(b * NMAX + t) * ld;
+    float2* col = tile[t];
     const float2* ta = tdiag + (size_t)i * NMAX;
     int rq = 0;
     for (int l = 1; l <= LMAX; ++l)
@@ -121,6 +123,12 @@ __global__ void __launch_bounds__(kAsmThreads) assemble_blocks_kernel(
                 col[tau * H + rq] = make_float2(-(q.x * w.x - q.y * w.y), -(q.x * w.y + q.y * w.x));   // a != b: no delta
             }
         }
+    }
+    __syncthreads();
+    for (int e = t; e < NMAX * NMAX; e += kAsmThreads) {   // consecutive threads, consecutive rows of one column
+        const int c = e / NMAX, n = e - c * NMAX;
+        out[(size_t)c * ld + n] = tile[c][n];
+    }
 }
 
 // z = blockdiag(Minv_j) v.  CTA c handles rows [row0, row0 + kGemvRows) of subset cta_group[c]; one thread per row,

@@ -341,6 +341,43 @@ def test_block_inversion_needs_and_survives_row_interchanges(N):
     assert rel(back, b) <= SOLVE_TOL
 
 
+@pytest.mark.parametrize("lmax", [1, 4])
+def test_block_inversion_degenerate_cases(lmax):
+    """Edge cases of the batched elimination (csrc/block_inverse.cuh).  (a) Cuboids so small that every sphere is alone:
+    every block is the identity (W^{ii} = 0), narrower than one 32-column panel at lmax = 1 (n = 6) and one full + one
+    ragged panel at lmax = 4 (n = 48); the apply must return v EXACTLY.  (b) A second set-up replaces the first and
+    matches the oracle for ITS cuboids.  (c) Aliased or missing arguments and a subset above 25600 / nmax spheres are
+    CELES_EINVAL, and the context stays usable."""
+    import dataclasses
+    w = dataclasses.replace(workloads.scaled(workloads.C2, 90), lmax=lmax)
+    pos, rad, q, ctx, b = make(w)
+    bd = torch.from_numpy(b).cuda()
+    with pytest.raises(celes.CelesError):
+        celes.celes_precond_apply(ctx, bd)                           # no preconditioner yet
+    info = celes.celes_precond_setup(ctx, 1.0)                       # 1 nm cuboids: singletons
+    assert info["n_groups"] == w.N and info["max_group_spheres"] == 1
+    assert info["block_bytes"] == 8 * w.N * w.nmax ** 2
+    z = celes.celes_precond_apply(ctx, bd)
+    assert torch.equal(torch.view_as_real(z), torch.view_as_real(bd))
+    with pytest.raises(celes.CelesError):
+        celes.celes_precond_apply(ctx, bd, bd)                       # v and z must not alias
+    qo = orc.mie_q(w.lmax, w.k, rad, workloads.N_SPHERE)
+    for edge in ([700.0, 0.0, 450.0], 1100.0):                       # (b): replaced twice, blocks of very different sizes
+        info = celes.celes_precond_setup(ctx, edge)
+        groups = orc.cuboid_partition(pos, edge)
+        assert info["n_groups"] == len(groups) and info["max_group_spheres"] == max(len(g) for g in groups)
+        assert min(len(g) for g in groups) < max(len(g) for g in groups)
+        z = celes.celes_precond_apply(ctx, bd).cpu().numpy()
+        assert rel(z, orc.precond_apply(pos, w.k, w.lmax, qo, edge, b)) <= SOLVE_TOL
+    if lmax == 4:                                                    # (c) 600 x 48 = 28800 rows in one subset
+        wl = workloads.scaled(workloads.C5, 600)
+        _, _, _, big, _ = make(wl)
+        with pytest.raises(celes.CelesError) as e:
+            celes.celes_precond_setup(big, 0.0)
+        assert e.value.code == celes.CELES_EINVAL
+        celes.celes_precond_setup(big, 600.0)                        # still usable
+
+
 def test_preconditioned_solve_same_solution_fewer_iterations():
     """Right-preconditioned GMRES: same solution as the oracle's tight solve, fewer iterations
     than the unpreconditioned solve; asking for the preconditioner before celes_precond_setup is an error."""

@@ -41,7 +41,7 @@ FP32_LANES_PER_SM = 128
 PRECOND_EDGE_NM = 600.0     # lateral cuboid edge of the preconditioned config-5 solve in the default line
 # dram__bytes_read.sum + dram__bytes_write.sum of one coupling-kernel launch, from the ncu --set full capture
 # summarised in the named file under profiles/ (a capture, not a live measurement: ncu cannot run inside the timed run)
-NCU_DRAM_BYTES_PER_LAUNCH = {("C4", "rotated"): (57.2e6, "profiles/r02b_kernel_c4.md")}
+NCU_DRAM_BYTES_PER_LAUNCH = {("C4", "rotated"): (87.3e6, "profiles/r02i_kernel_c4.md")}
 
 
 def parse():

@@ -12,13 +12,19 @@
 //       free up, so the short runs at the end even out what the long ones leave uneven -- and they leave a lot: of two
 //       CTAs resident on an SM the warp scheduler favours one almost exclusively (measured: it finishes after 58 % of the
 //       pair's time, profiles/r02_cta_trace.md), and a CTA left alone on an SM reaches only 92 % of the pipe throughput
-//       of two.  One level (a single wave of equal runs) is 5.5 % slower than many waves for that reason, six levels are
-//       within 0.2 %, with n_res * levels + rblocks partial sums instead of 56 per receiver block at N = 1e4.
+//       of two.  One level (a single wave of equal runs) is 5.5 % slower than many waves for that reason; at N = 1e5
+//       six levels take 357.25 ms, ten (the default) 355.90 ms and more change nothing; at N = 1e4 the halving stops after
+//       five levels whatever is asked (runs shorter than CELES_MIN_RUN_TILES tiles are not made: shorter ones were
+//       measured slower).  At most n_res * levels + rblocks partial sums, instead of 56 per receiver block at N = 1e4.
 //   fixed splits (celes_options.emitter_splits = S > 0): every block's emitters are cut into S equal chunks, one CTA
 //       each, grid = rblocks x S CTAs in as many waves as that takes.
 #pragma once
 #include <algorithm>
 #include <vector>
+
+#ifndef CELES_MIN_RUN_TILES
+#define CELES_MIN_RUN_TILES 4     // shortest run the halving may produce, in emitter tiles
+#endif
 
 namespace celes {
 
@@ -56,7 +62,7 @@ inline WorkPartition build_partition(int N, int kblock, int etile, int n_res, in
         for (int lev = 0; lev < std::max(1, levels) && done < total; ++lev) {
             const bool last = lev + 1 >= std::max(1, levels);
             long long share = last ? total - done : (total - done) / 2;
-            if (share < 4LL * n_res) share = total - done;             // runs of a few tiles: stop halving
+            if (share < (long long)CELES_MIN_RUN_TILES * n_res) share = total - done;   // runs of a few tiles: stop halving
             const long long n = std::max<long long>(1, std::min<long long>(n_res, share));
             for (long long c = 0; c < n; ++c) {
                 const long long a = done + share * c / n, b = done + share * (c + 1) / n;

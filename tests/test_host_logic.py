@@ -213,7 +213,7 @@ def test_work_partition_covers_every_pair_once(N, etile, res, levels, splits):
     tiles = np.zeros(p["ctas"], dtype=np.int64)
     np.add.at(tiles, seg[:, 0], -(-(seg[:, 3] - seg[:, 2]) // etile))
     if splits == 0:
-        lv = levels or 6
+        lv = levels or 10                                               # CELES_DEFAULT_LEVELS
         assert p["ctas"] <= res * lv and len(seg) <= p["ctas"] + rblocks * lv
         assert np.all(np.diff(tiles) <= 1)                              # runs never grow along the launch order
         if levels == 1:

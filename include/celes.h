@@ -172,7 +172,7 @@ int celes_solve(celes_ctx* ctx, const void* a_in_dev, void* x_dev, const celes_s
  * is assembled on the device and eliminated with partial (row) pivoting through to its inverse (a blocked Gauss-Jordan
  * elimination in the library's own kernels, all blocks side by side); the context stores the inverses
  * (8 * sum_j (N_j nmax)^2 bytes; the elimination runs in place).  Replaces an earlier preconditioner of
- * the context, reusing its block buffer if the new blocks fit.  Synchronises.
+ * the context, reusing its device memory if the new one fits (no allocator call then).  Synchronises the device.
  * CELES_EINVAL: bad argument or a subset with more than 25600 / nmax spheres; CELES_ENOMEM: blocks do not fit;
  * CELES_ECUDA: CUDA failure or a singular block. */
 int celes_precond_setup(celes_ctx* ctx, const double* edge_xyz, celes_precond_info* info, void* cuda_stream);

@@ -52,6 +52,8 @@ struct celes_ctx {
     int pc_groups = 0, pc_max_n = 0, pc_ctas = 0;
     long long pc_elems = 0;      // sum_j n_j^2
     long long pc_capacity = 0;   // elements allocated behind pc_blocks (a later set-up that fits reuses the buffer)
+    char* pc_arena = nullptr;    // one allocation behind every index / work array of the preconditioner (and the set-up's
+    size_t pc_arena_bytes = 0;   // temporaries): grow-only, so a set-up that replaces an earlier one calls no allocator
     int* pc_order = nullptr;     // [N]
     int* pc_grp_offset = nullptr;        // [groups+1]
     long long* pc_blk_offset = nullptr;  // [groups]

@@ -16,12 +16,17 @@
 #include "precond_kernels.cuh"
 #include "translation_table.h"
 
-void celes::host::free_precond(celes_ctx* c) {
-    cudaFree(c->pc_order); cudaFree(c->pc_grp_offset); cudaFree(c->pc_blk_offset); cudaFree(c->pc_cta_group);
-    cudaFree(c->pc_cta_row0); cudaFree(c->pc_perm); cudaFree(c->pc_blocks); cudaFree(c->pc_tmp);
+// the preconditioner's arrays are pieces of pc_arena; pc_blocks is its own allocation
+static void forget_precond(celes_ctx* c) {
     c->pc_order = c->pc_grp_offset = c->pc_cta_group = c->pc_cta_row0 = c->pc_perm = nullptr;
-    c->pc_blk_offset = nullptr; c->pc_blocks = c->pc_tmp = nullptr;
-    c->pc_ready = false; c->pc_groups = c->pc_max_n = c->pc_ctas = 0; c->pc_elems = 0; c->pc_capacity = 0;
+    c->pc_blk_offset = nullptr; c->pc_tmp = nullptr;
+    c->pc_ready = false; c->pc_groups = c->pc_max_n = c->pc_ctas = 0; c->pc_elems = 0;
+}
+
+void celes::host::free_precond(celes_ctx* c) {
+    cudaFree(c->pc_arena); cudaFree(c->pc_blocks);
+    c->pc_arena = nullptr; c->pc_arena_bytes = 0; c->pc_blocks = nullptr; c->pc_capacity = 0;
+    forget_precond(c);
 }
 
 // z = blockdiag(M_j^{-1}) v  (step 4)
@@ -67,15 +72,18 @@ int celes_partition(int N, const double* pos_xyz, const double* edge_xyz, int* g
 // batched matrix-vector product (block_gemv_kernel).
 static int precond_setup_impl(celes_ctx* ctx, const double* edge_xyz, celes_precond_info* info, cudaStream_t s) {
     const auto t_start = std::chrono::steady_clock::now();
-    // a set-up that replaces an earlier one keeps the block buffer if the new blocks fit (no GB-sized free + allocation)
-    float2* kept = ctx->pc_blocks;
-    const long long kept_capacity = ctx->pc_capacity;
-    ctx->pc_blocks = nullptr;
-    free_precond(ctx);
-    ctx->pc_blocks = kept; ctx->pc_capacity = kept_capacity;         // owned by the context again: every exit path frees or keeps it
+    const bool dbg = std::getenv("CELES_DEBUG") != nullptr;
+    auto since = [&]() { return std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t_start).count(); };
+    double t_free0 = 0, t_part = 0, t_tables = 0, t_alloc = 0, t_h2d = 0, t_gpu = 0;
+    // a set-up that replaces an earlier one keeps the block buffer and the arena if the new preconditioner fits: it then
+    // calls no allocator at all (cudaMalloc / cudaFree were measured at 1 ms ... 140 ms per set-up, unpredictably)
+    if (ctx->pc_ready && cudaDeviceSynchronize() != cudaSuccess) return CELES_ECUDA;   // nothing may still read the arrays about to be rewritten
+    forget_precond(ctx);
+    t_free0 = since();
     celes::Partition part;
     if (!celes::build_partition(ctx->N, ctx->pos.data(), edge_xyz, part)) return CELES_EINVAL;
     const int G = part.n_groups(), nmax = ctx->nmax;
+    t_part = since();
     const long long max_n = (long long)part.max_group() * nmax;
     if (max_n * (long long)sizeof(float2) > 200 * 1024) return CELES_EINVAL;      // subset too large for one CTA's x slice
     std::vector<long long> blk_off(G), pair_off(G + 1, 0);
@@ -103,13 +111,12 @@ static int precond_setup_impl(celes_ctx* ctx, const double* edge_xyz, celes_prec
     std::vector<double> a5d, b5d;
     if (!celes::build_translation_table(ctx->lmax, a5d, b5d)) return CELES_EINVAL;
     std::vector<float> a5f(a5d.begin(), a5d.end()), b5f(b5d.begin(), b5d.end());
+    t_tables = since();
 
     long long *d_pair_off = nullptr, *d_tile_off = nullptr;
     float *d_a5 = nullptr, *d_b5 = nullptr;
     int *d_info = nullptr, *d_by_size = nullptr, *d_src_row = nullptr, *d_disp_count = nullptr, *d_disp_rows = nullptr;
     auto cleanup = [&](int code) {
-        cudaFree(d_pair_off); cudaFree(d_tile_off); cudaFree(d_a5); cudaFree(d_b5); cudaFree(d_info);
-        cudaFree(d_by_size); cudaFree(d_src_row); cudaFree(d_disp_count); cudaFree(d_disp_rows);
         if (code != CELES_OK) free_precond(ctx);
         return code;
     };
@@ -122,28 +129,34 @@ static int precond_setup_impl(celes_ctx* ctx, const double* edge_xyz, celes_prec
         }                                                                                              \
     } while (0)
     const size_t rows = (size_t)ctx->N * nmax;
-    PC_TRY(cudaMalloc(&ctx->pc_order, sizeof(int) * ctx->N));
-    PC_TRY(cudaMalloc(&ctx->pc_grp_offset, sizeof(int) * (G + 1)));
-    PC_TRY(cudaMalloc(&ctx->pc_blk_offset, sizeof(long long) * G));
-    PC_TRY(cudaMalloc(&ctx->pc_cta_group, sizeof(int) * cta_group.size()));
-    PC_TRY(cudaMalloc(&ctx->pc_cta_row0, sizeof(int) * cta_row0.size()));
-    PC_TRY(cudaMalloc(&ctx->pc_perm, sizeof(int) * rows));
+    // every array but the blocks is a 256-byte aligned piece of one arena (persistent tables first, temporaries after)
+    size_t arena_need = 0;
+    auto piece = [&](size_t bytes) { const size_t at = arena_need; arena_need += (bytes + 255) & ~(size_t)255; return at; };
+    const size_t o_order = piece(sizeof(int) * ctx->N), o_grp = piece(sizeof(int) * (G + 1)), o_blk = piece(sizeof(long long) * G),
+                 o_ctag = piece(sizeof(int) * cta_group.size()), o_ctar = piece(sizeof(int) * cta_row0.size()),
+                 o_perm = piece(sizeof(int) * rows), o_tmp = piece(sizeof(float2) * rows), o_src = piece(sizeof(int) * rows),
+                 o_pair = piece(sizeof(long long) * (G + 1)), o_tile = piece(sizeof(long long) * (G + 1)),
+                 o_a5 = piece(sizeof(float) * a5f.size()), o_b5 = piece(sizeof(float) * b5f.size()), o_info = piece(sizeof(int) * (size_t)G),
+                 o_dc = piece(sizeof(int) * (size_t)G), o_dr = piece(sizeof(int) * (size_t)G * celes::kGjNb), o_bs = piece(sizeof(int) * (size_t)G);
+    if (ctx->pc_arena_bytes < arena_need) {
+        cudaFree(ctx->pc_arena);
+        ctx->pc_arena = nullptr; ctx->pc_arena_bytes = 0;
+        PC_TRY(cudaMalloc(&ctx->pc_arena, arena_need));
+        ctx->pc_arena_bytes = arena_need;
+    }
     if (ctx->pc_capacity < elems) {
         cudaFree(ctx->pc_blocks);
         ctx->pc_blocks = nullptr; ctx->pc_capacity = 0;
         PC_TRY(cudaMalloc(&ctx->pc_blocks, sizeof(float2) * (size_t)elems));
         ctx->pc_capacity = elems;
     }
-    PC_TRY(cudaMalloc(&ctx->pc_tmp, sizeof(float2) * rows));
-    PC_TRY(cudaMalloc(&d_src_row, sizeof(int) * rows));
-    PC_TRY(cudaMalloc(&d_pair_off, sizeof(long long) * (G + 1)));
-    PC_TRY(cudaMalloc(&d_tile_off, sizeof(long long) * (G + 1)));
-    PC_TRY(cudaMalloc(&d_a5, sizeof(float) * a5f.size()));
-    PC_TRY(cudaMalloc(&d_b5, sizeof(float) * b5f.size()));
-    PC_TRY(cudaMalloc(&d_info, sizeof(int) * (size_t)G));
-    PC_TRY(cudaMalloc(&d_disp_count, sizeof(int) * (size_t)G));
-    PC_TRY(cudaMalloc(&d_disp_rows, sizeof(int) * (size_t)G * celes::kGjNb));
-    PC_TRY(cudaMalloc(&d_by_size, sizeof(int) * (size_t)G));
+    char* A = ctx->pc_arena;
+    ctx->pc_order = (int*)(A + o_order); ctx->pc_grp_offset = (int*)(A + o_grp); ctx->pc_blk_offset = (long long*)(A + o_blk);
+    ctx->pc_cta_group = (int*)(A + o_ctag); ctx->pc_cta_row0 = (int*)(A + o_ctar); ctx->pc_perm = (int*)(A + o_perm);
+    ctx->pc_tmp = (float2*)(A + o_tmp); d_src_row = (int*)(A + o_src); d_pair_off = (long long*)(A + o_pair);
+    d_tile_off = (long long*)(A + o_tile); d_a5 = (float*)(A + o_a5); d_b5 = (float*)(A + o_b5); d_info = (int*)(A + o_info);
+    d_disp_count = (int*)(A + o_dc); d_disp_rows = (int*)(A + o_dr); d_by_size = (int*)(A + o_bs);
+    t_alloc = since();
     PC_TRY(cudaMemcpyAsync(ctx->pc_order, part.order.data(), sizeof(int) * ctx->N, cudaMemcpyHostToDevice, s));
     PC_TRY(cudaMemcpyAsync(ctx->pc_grp_offset, part.offset.data(), sizeof(int) * (G + 1), cudaMemcpyHostToDevice, s));
     PC_TRY(cudaMemcpyAsync(ctx->pc_blk_offset, blk_off.data(), sizeof(long long) * G, cudaMemcpyHostToDevice, s));
@@ -155,6 +168,7 @@ static int precond_setup_impl(celes_ctx* ctx, const double* edge_xyz, celes_prec
     PC_TRY(cudaMemcpyAsync(d_b5, b5f.data(), sizeof(float) * b5f.size(), cudaMemcpyHostToDevice, s));
     PC_TRY(cudaMemcpyAsync(d_by_size, by_size.data(), sizeof(int) * (size_t)G, cudaMemcpyHostToDevice, s));
     PC_TRY(cudaMemsetAsync(d_info, 0, sizeof(int) * (size_t)G, s));
+    t_h2d = since();
     // (2) assemble every block
     {
         const unsigned grid = (unsigned)pair_off[G];
@@ -196,6 +210,7 @@ static int precond_setup_impl(celes_ctx* ctx, const double* edge_xyz, celes_prec
     std::vector<int> infos((size_t)G);
     PC_TRY(cudaMemcpyAsync(infos.data(), d_info, sizeof(int) * infos.size(), cudaMemcpyDeviceToHost, s));
     PC_TRY(cudaStreamSynchronize(s));
+    t_gpu = since();
 #undef PC_TRY
     for (int v : infos)
         if (v != 0) {                                                // singular block
@@ -210,7 +225,11 @@ static int precond_setup_impl(celes_ctx* ctx, const double* edge_xyz, celes_prec
         info->block_bytes = elems * (long long)sizeof(float2);
         info->seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_start).count();
     }
-    return cleanup(CELES_OK);
+    const int rc_done = cleanup(CELES_OK);
+    if (dbg)
+        std::fprintf(stderr, "celes_precond_setup ms: free-old %.2f | partition %.2f | tables %.2f | alloc %.2f | h2d %.2f | gpu %.2f | free-tmp %.2f (cumulative)\n",
+                     t_free0, t_part, t_tables, t_alloc, t_h2d, t_gpu, since());
+    return rc_done;
 }
 
 int celes_precond_setup(celes_ctx* ctx, const double* edge_xyz, celes_precond_info* info, void* cuda_stream) {

@@ -508,6 +508,8 @@ def solve_c5(celes, fields, workloads, translation, precond_edge=0.0):
            "converged": bool(info["converged"])}
     if pc is not None:
         out["preconditioner"] = dict(pc, edge_nm=precond_edge, setup_seconds=t_setup,
+                                     setup_note="replaces a warm-up set-up on the same context: device memory is reused, no "
+                                                "allocator call; a context's first set-up adds its allocations (2-22 ms seen)",
                                      apply_roofline=precond_apply_roofline(celes, ctx, a_in, pc))
     return out, ctx, a_in
 

@@ -60,6 +60,8 @@ def parse():
                     help="time celes_far_field on NB x 2NB directions (Gauss-Legendre x uniform azimuth) instead")
     ap.add_argument("--near-field", type=int, default=0, metavar="NP",
                     help="time celes_scattered_field on an NP x NP grid of points in the plane 300 nm above the slab instead")
+    ap.add_argument("--gaussian-beam", action="store_true",
+                    help="time celes_gaussian_beam (waist 4 um, PAPER.md:140, centred on the slab, normal incidence) instead")
     ap.add_argument("--lmax", type=int, default=0, help="override the workload's truncation order (1..5)")
     ap.add_argument("--hankel", default="registers", choices=["registers", "table"],
                     help="h_p(kd) in registers (default) or from the paper's lookup table (PAPER.md:130)")
@@ -316,6 +318,36 @@ def run_far_field(args, w):
                      "fma_pipe_utilisation_whole_call": lane * terms / sec / (FP32_LANES_PER_SM * sm * device_sm_clock_hz())}}))
 
 
+def run_gaussian_beam(args, w):
+    """celes_gaussian_beam (Appendix C, (C.7)-(C.8)): initial-field coefficients of the paper's beam (waist 4 um,
+    PAPER.md:140) for every sphere of the workload; FP64 input preparation, once per simulation."""
+    import torch
+    import paper_1706_02145_b200 as celes
+    from paper_1706_02145_b200 import fields, workloads
+    torch.cuda.set_device(0)
+    pos, rad = workloads.positions(w)
+    q = fields.mie_coefficients(w.lmax, w.k, rad, workloads.N_SPHERE)
+    ctx = celes.celes_setup(pos, rad, q, w.k, w.lmax)
+    centre = [0.0, 0.0, float(pos[:, 2].min()) - 200.0]
+    a_in = torch.empty(w.N, w.nmax, dtype=torch.complex64, device="cuda")
+    for _ in range(max(2, args.warmup)):
+        celes.celes_gaussian_beam(ctx, 4000.0, centre, a_in=a_in)
+    times = []
+    for _ in range(max(1, args.steps)):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        celes.celes_gaussian_beam(ctx, 4000.0, centre, a_in=a_in)
+        e1.record()
+        torch.cuda.synchronize()
+        times.append(e0.elapsed_time(e1) * 1e-3)
+    sec = float(np.median(times))
+    print(json.dumps({
+        "metric": "beam_coefficients_per_s", "value": w.N * w.nmax / sec, "unit": "coefficients/s", "n_gpus": 1,
+        "steps": len(times), "ms_per_call": sec * 1e3, "higher_is_better": True, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"{w.name}: N={w.N} lmax={w.lmax}", "waist_nm": 4000.0,
+                   "norm_a_in": float(torch.linalg.vector_norm(a_in))}}))
+
+
 def run_sharded(args, w):
     """--gpus N --shard receivers under torchrun: every rank owns a slice of the receiver rows (and of b); a step is one
     all-gather of b (NCCL) + celes_coupling_matvec_rows on the rank's rows.  value = N (N - 1) / slowest rank's time:
@@ -532,6 +564,9 @@ def main():
         return
     if args.near_field > 0:
         run_near_field(args, w)
+        return
+    if args.gaussian_beam:
+        run_gaussian_beam(args, w)
         return
     if args.shard == "receivers":
         run_sharded(args, w)

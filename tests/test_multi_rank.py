@@ -95,3 +95,41 @@ def test_all_gather_of_row_shards_gloo_world2():
     out = json.loads([l for l in r.stdout.splitlines() if l.startswith("RESULT ")][0][7:])
     assert out["world"] == 2 and out["ok"] == [True, True]
     assert out["slices"] == [[0, 128], [128, 301]]
+
+
+REFERENCE_KEYS = {"impl", "metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
+                  "vs_baseline", "dtype", "data", "config", "cpu_baseline", "e2e", "gpu_launches"}
+
+
+def _check_reference_line(line: dict, n_gpus: int):
+    assert REFERENCE_KEYS <= set(line) and line["impl"] == "reference"
+    assert line["metric"] == "sphere_pair_translations_per_s" and line["unit"] == "pairs/s" and line["higher_is_better"] is True
+    assert line["n_gpus"] == n_gpus and line["steps"] == 1 and line["value"] > 0 and line["gpu_launches"] == 0
+    assert line["cpu_baseline"]["kind"] == "oracle" and line["cpu_baseline"]["cores"] >= 1
+    assert line["cpu_baseline"]["value"] == line["value"] and "receivers" in line["cpu_baseline"]["sample"]
+    assert line["e2e"] == {"value": line["value"], "unit": "pairs/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
+    assert "workload" in line["config"] and "model" not in line["config"]
+
+
+def test_reference_arm_prints_the_contract_line_without_a_gpu():
+    """bench.py --impl reference: the oracle, as it stands, on the host cores (the tier's reference arm); runs anywhere,
+    prints exactly one JSON line with the arm's keys.  Config 1 (N = 50) keeps it to a second."""
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--workload", "C1",
+                        "--steps", "1", "--warmup", "0"], cwd=ROOT, capture_output=True, text=True, timeout=300)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [l for l in r.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1
+    _check_reference_line(json.loads(lines[0]), 1)
+
+
+def test_reference_arm_under_torchrun_only_rank0_works():
+    """Launched like the GPU arm for N = 2 (torchrun, two ranks): rank 0 alone runs and prints, rank 1 exits 0 silently."""
+    env = dict(os.environ, PYTHONPATH=ROOT)
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node=2", "--master-addr", "127.0.0.1",
+           "--master-port", "29617", os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2", "--workload", "C1",
+           "--steps", "1", "--warmup", "0"]
+    r = subprocess.run(cmd, env=env, cwd=ROOT, capture_output=True, text=True, timeout=300)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [l for l in r.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1
+    _check_reference_line(json.loads(lines[0]), 2)

@@ -84,6 +84,31 @@ def test_overlap_check_finds_a_single_overlap_in_a_large_packing():
     assert _setup_rc(w.N, w.lmax, bad, rad, q, w.k)[0] == binding.CELES_EINVAL
 
 
+def test_without_a_gpu_the_product_fails_loudly_and_never_touches_the_oracle():
+    """No CPU fallback (the tier's rule): on a box without a CUDA device a valid celes_setup is CELES_ECUDA and returns no
+    context, bench.py's own arm exits non-zero saying so, and importing the product (package + bench) imports nothing of
+    oracle/.  Skipped where a GPU is present (the GPU tests cover that side)."""
+    import subprocess
+    import sys
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a CUDA device is present")
+    w = workloads.C1
+    pos, rad = workloads.positions(w)
+    rc, handle = _setup_rc(w.N, w.lmax, pos, rad, np.zeros((w.N, 2, w.lmax), complex), w.k)
+    assert rc == binding.CELES_ECUDA and not handle
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--steps", "1", "--warmup", "0"], cwd=ROOT,
+                       capture_output=True, text=True, timeout=300)
+    assert r.returncode != 0 and "no CPU fallback" in (r.stderr + r.stdout)
+    assert not [l for l in r.stdout.splitlines() if l.startswith("{")]            # and no number is printed
+    code = ("import sys; sys.path.insert(0, %r); import paper_1706_02145_b200, bench; "
+            "from paper_1706_02145_b200 import binding, fields, workloads, sharding, sass_count; "
+            "bad = [m for m in sys.modules if m == 'oracle' or m.startswith('oracle.')]; print('ORACLE', bad)" % ROOT)
+    r = subprocess.run([sys.executable, "-c", code], cwd=ROOT, capture_output=True, text=True, timeout=300)
+    assert r.returncode == 0, r.stderr[-1500:]
+    assert "ORACLE []" in r.stdout
+
+
 def test_compute_entry_points_reject_null():
     L = binding.lib()
     assert L.celes_coupling_matvec(None, None, None, None) == binding.CELES_EINVAL

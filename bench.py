@@ -66,6 +66,7 @@ def parse():
     ap.add_argument("--hankel", default="registers", choices=["registers", "table"],
                     help="h_p(kd) in registers (default) or from the paper's lookup table (PAPER.md:130)")
     ap.add_argument("--method", default="gmres", choices=["gmres", "bicgstab"], help="with --solve")
+    ap.add_argument("--restart", type=int, default=30, help="with --solve: GMRES restart length (BASELINE config 5: 30)")
     ap.add_argument("--cta-trace", action="store_true",
                     help="per-CTA start / end times and SM of the coupling kernel for --levels 1 and the default partition "
                          "(needs a library built with CELES_NVCC_EXTRA=-DCELES_TRACE python -m paper_1706_02145_b200.build --force)")
@@ -248,7 +249,7 @@ def run_solve(args, w):
     ctx = celes.celes_setup(pos, rad, q, w.k, w.lmax, translation=args.translation)
     a_in = torch.from_numpy(fields.plane_wave_coefficients(pos, w.k, w.lmax).astype(np.complex64)).cuda()
     x = torch.zeros(w.N, w.nmax, dtype=torch.complex64, device="cuda")
-    celes.celes_solve(ctx, a_in, x, restart=30, rtol=1e-4, max_iters=3)          # warm-up (allocations, caches)
+    celes.celes_solve(ctx, a_in, x, restart=args.restart, rtol=1e-4, max_iters=3)          # warm-up (allocations, caches)
     pc = None
     if args.precond_edge > 0:
         celes.celes_precond_setup(ctx, [args.precond_edge, args.precond_edge, 0.0])   # warm-up (kernel load)
@@ -259,7 +260,7 @@ def run_solve(args, w):
         t0 = time.perf_counter()
         if args.precond_edge > 0:                                                # set-up is part of the time to solution
             pc = celes.celes_precond_setup(ctx, [args.precond_edge, args.precond_edge, 0.0])
-        info = celes.celes_solve(ctx, a_in, x, restart=30, rtol=1e-4, max_iters=2000, precond=pc is not None,
+        info = celes.celes_solve(ctx, a_in, x, restart=args.restart, rtol=1e-4, max_iters=2000, precond=pc is not None,
                                  method=args.method)
         torch.cuda.synchronize()
         runs.append((time.perf_counter() - t0, info))
@@ -269,7 +270,7 @@ def run_solve(args, w):
     print(json.dumps({
         "metric": "time_to_solution_s", "value": float(np.median(secs)), "unit": "s", "n_gpus": 1, "steps": len(runs),
         "warmup": 1, "higher_is_better": False, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": f"{w.name}: N={w.N} lmax={w.lmax} plane wave +z x-pol, GMRES(30) rtol 1e-4",
+        "config": {"workload": f"{w.name}: N={w.N} lmax={w.lmax} plane wave +z x-pol, GMRES({args.restart}) rtol 1e-4",
                    "translation": args.translation, "method": args.method,
                    "preconditioner": None if pc is None else dict(pc, edge_nm=args.precond_edge)},
         "precond_apply_roofline": pc_line,

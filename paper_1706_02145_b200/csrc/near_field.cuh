@@ -16,11 +16,6 @@ namespace celes {
 constexpr int kNearThreads = 128;
 constexpr int kNearTile = 32;
 
-__device__ __forceinline__ float2 cmul(float2 a, float2 b) { return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
-__device__ __forceinline__ float2 cscale(float s, float2 a) { return make_float2(s * a.x, s * a.y); }
-__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
-__device__ __forceinline__ float2 cmuli(float2 a) { return make_float2(-a.y, a.x); }     // i a
-
 // kpts [n_pts][3] FP64 = k r (dimensionless, like kpos); E [n_pts][3] complex64 (x, y, z components)
 template <int LMAX>
 __global__ void __launch_bounds__(kNearThreads) near_field_kernel(int N, int n_pts, const double* __restrict__ kpos,
@@ -56,13 +51,10 @@ __global__ void __launch_bounds__(kNearThreads) near_field_kernel(int N, int n_p
             float sx, cx;
             sincos_kd(x, 0.0f, &sx, &cx);
             float2 h[LMAX + 1];
-            h[0] = make_float2(sx * rinv, -cx * rinv);
-            h[1] = make_float2(fmaf(sx, rinv, -cx) * rinv, -fmaf(cx, rinv, sx) * rinv);
+            h[0] = mul2(bc2(rinv), make_float2(sx, -cx));
+            h[1] = fma2(bc2(rinv), h[0], nimul2(h[0]));             // h_1 = h_0 / x - e^{ix} / x,  e^{ix} / x = i h_0
 #pragma unroll
-            for (int l = 1; l < LMAX; ++l) {
-                const float f = (float)(2 * l + 1) * rinv;
-                h[l + 1] = make_float2(fmaf(f, h[l].x, -h[l - 1].x), fmaf(f, h[l].y, -h[l - 1].y));
-            }
+            for (int l = 1; l < LMAX; ++l) h[l + 1] = fma2(bc2((float)(2 * l + 1) * rinv), h[l], neg2(h[l - 1]));
             // normalised P_l^m and pi_l^m = P_l^m / sin(theta) (no division: started from P_{m-1}^{m-1})
             float P[LMAX + 1][LMAX + 1], pi[LMAX + 1][LMAX + 1];
 #pragma unroll
@@ -93,38 +85,46 @@ __global__ void __launch_bounds__(kNearThreads) near_field_kernel(int N, int n_p
             float2 ph[LMAX + 1];                                   // e^{i m phi}
             ph[0] = make_float2(1.f, 0.f);
 #pragma unroll
-            for (int m = 1; m <= LMAX; ++m) ph[m] = cmul(ph[m - 1], make_float2(cph, sph));
+            for (int m = 1; m <= LMAX; ++m) ph[m] = cmul2(make_float2(cph, sph), ph[m - 1]);
             const float2* be = sb + e * NMAX;
             float2 Er = make_float2(0.f, 0.f), Et = Er, Ep = Er;   // components along e_r, e_theta, e_phi of the pair
+            // (A.2): Psi_1 = u (i m pi e_theta - tau e_phi),  Psi_2 = v (l(l+1) h_l / x P e_r + dh (tau e_theta + i m pi e_phi)),
+            // u = nrm e^{i m phi} b_1 h_l, v = nrm e^{i m phi} b_2.  The radial factors depend on l only: the five angular sums
+            // over m are formed first (packed: one FFMA2 per real coefficient x complex value) and meet h_l, dh, h_l / x once per l.
 #pragma unroll
             for (int l = 1; l <= LMAX; ++l) {
                 const float nrm = rsqrtf(2.0f * l * (l + 1.0f));
                 const float2 hl = h[l];
                 // d(x h_l)/dx / x = h_{l-1} - l h_l / x
-                const float2 dh = make_float2(fmaf(-(float)l * rinv, hl.x, h[l - 1].x), fmaf(-(float)l * rinv, hl.y, h[l - 1].y));
-                const float2 hr = cscale((float)(l * (l + 1)) * rinv, hl);
+                const float2 dh = fma2(bc2(-(float)l * rinv), hl, h[l - 1]);
+                const float2 hlN = mul2(bc2(nrm), hl), dhN = mul2(bc2(nrm), dh), hrN = mul2(bc2(nrm * (float)(l * (l + 1)) * rinv), hl);
+                float2 S1 = make_float2(0.f, 0.f), S2 = S1, T1 = S1, T2 = S1, T3 = S1;
 #pragma unroll
                 for (int m = -l; m <= l; ++m) {
                     const int am = m < 0 ? -m : m;
                     const float tau = am == 0 ? -sqrtf((float)(l * (l + 1))) * P[l][1]
                                               : l * ct * pi[l][am] - (l + am) * sqrtf((2.0f * l + 1.0f) / (2.0f * l - 1.0f) * (float)(l - am) / (float)(l + am)) * (l - 1 >= am ? pi[l - 1][am] : 0.0f);
-                    const float mpi = (float)m * pi[l][am];
                     const float2 phase = m < 0 ? make_float2(ph[am].x, -ph[am].y) : ph[am];
                     const int q = (l - 1) * (l + 1) + (m + l);
-                    const float2 pref = cscale(nrm, phase);
-                    const float2 u = cmul(cmul(pref, be[q]), hl);          // tau = 1: pref b h_l
-                    const float2 v = cmul(pref, be[H + q]);                // tau = 2: pref b
-                    const float2 vd = cmul(v, dh);
-                    // (A.2): Psi_1 = u (i m pi e_theta - tau e_phi);  Psi_2 = v (l(l+1) h_l / x P e_r + dh (tau e_theta + i m pi e_phi))
-                    Et = cadd(Et, cadd(cscale(mpi, cmuli(u)), cscale(tau, vd)));
-                    Ep = cadd(Ep, cadd(cscale(-tau, u), cscale(mpi, cmuli(vd))));
-                    Er = cadd(Er, cscale(P[l][am], cmul(v, hr)));
+                    const float2 c1 = m == 0 ? be[q] : cmul2(phase, be[q]);           // e^{i m phi} b_1
+                    const float2 c2 = m == 0 ? be[H + q] : cmul2(phase, be[H + q]);   // e^{i m phi} b_2
+                    S2 = fma2(bc2(-tau), c1, S2);
+                    T1 = fma2(bc2(tau), c2, T1);
+                    T3 = fma2(bc2(P[l][am]), c2, T3);
+                    if (m != 0) {
+                        const float mpi = (float)m * pi[l][am];
+                        S1 = fma2(bc2(mpi), imul2(c1), S1);
+                        T2 = fma2(bc2(mpi), imul2(c2), T2);
+                    }
                 }
+                Et = cfma2(dhN, T1, cfma2(hlN, S1, Et));
+                Ep = cfma2(dhN, T2, cfma2(hlN, S2, Ep));
+                Er = cfma2(hrN, T3, Er);
             }
             // e_r = (st cph, st sph, ct), e_theta = (ct cph, ct sph, -st), e_phi = (-sph, cph, 0)
-            Ex = cadd(Ex, cadd(cadd(cscale(st * cph, Er), cscale(ct * cph, Et)), cscale(-sph, Ep)));
-            Ey = cadd(Ey, cadd(cadd(cscale(st * sph, Er), cscale(ct * sph, Et)), cscale(cph, Ep)));
-            Ez = cadd(Ez, cadd(cscale(ct, Er), cscale(-st, Et)));
+            Ex = fma2(bc2(-sph), Ep, fma2(bc2(ct * cph), Et, fma2(bc2(st * cph), Er, Ex)));
+            Ey = fma2(bc2(cph), Ep, fma2(bc2(ct * sph), Et, fma2(bc2(st * sph), Er, Ey)));
+            Ez = fma2(bc2(-st), Et, fma2(bc2(ct), Er, Ez));
         }
     }
     if (active) {

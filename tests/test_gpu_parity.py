@@ -536,6 +536,46 @@ def test_solve_warm_start_from_x0():
     assert rel(rough.cpu().numpy(), x.cpu().numpy()) <= 1e-3
 
 
+_ENOCONV_REF = []
+
+
+def _enoconv_reference():
+    """The oracle's tight solve of the ensemble the test below uses, computed once for its four variants."""
+    if not _ENOCONV_REF:
+        w = workloads.scaled(workloads.C5, 300)
+        pos, rad = workloads.positions(w)
+        qo = orc.mie_q(w.lmax, w.k, rad, workloads.N_SPHERE)
+        a_in = orc.plane_wave_a_in(pos, w.k, w.lmax)
+        xref, _ = orc.solve_gmres(pos, w.k, w.lmax, qo, a_in, rtol=1e-10)
+        _ENOCONV_REF.append((w, pos, rad, a_in, qo, xref))
+    return _ENOCONV_REF[0]
+
+
+@pytest.mark.parametrize("method,precond", [("gmres", False), ("gmres", True), ("bicgstab", False), ("bicgstab", True)])
+def test_solve_out_of_iterations_reports_enoconv_with_x_and_info_filled(method, precond):
+    """include/celes.h: "Returns CELES_OK, or CELES_ENOCONV with x and info still filled".  With max_iters cut short the
+    call says not converged, the residual it reports is the TRUE residual of the x it returns (checked through an
+    independent system matvec), the history is monotone information about that run, and solving on from that x converges
+    to the oracle's solution."""
+    w, pos, rad, a_in, qo, xref = _enoconv_reference()
+    ctx = celes.celes_setup(pos, rad, fields.mie_coefficients(w.lmax, w.k, rad, workloads.N_SPHERE), w.k, w.lmax)
+    a_dev = torch.from_numpy(a_in.astype(np.complex64)).cuda()
+    if precond:
+        celes.celes_precond_setup(ctx, [900.0, 900.0, 0.0])
+    x = torch.zeros(w.N, w.nmax, dtype=torch.complex64, device="cuda")
+    short = celes.celes_solve(ctx, a_dev, x, restart=4, rtol=1e-4, max_iters=6, method=method, precond=precond)
+    assert short["code"] == celes.CELES_ENOCONV and not short["converged"]
+    assert 6 <= short["iterations"] <= 8 and short["matvecs"] >= short["iterations"]
+    assert 1e-4 < short["rel_residual"] < 1.0 and len(short["history"]) >= 1
+    rhs = orc.t_diagonal(qo, w.lmax) * a_in
+    res = rhs - celes.celes_system_matvec(ctx, x).cpu().numpy()
+    true_rel = float(np.linalg.norm(res) / np.linalg.norm(rhs))
+    assert abs(true_rel - short["rel_residual"]) <= 2e-3 * true_rel + 1e-6
+    more = celes.celes_solve(ctx, a_dev, x, restart=30, rtol=1e-4, max_iters=2000, method=method, precond=precond)
+    assert more["code"] == celes.CELES_OK and more["converged"] and more["rel_residual"] <= 1e-4
+    assert rel(x.cpu().numpy(), xref) <= SOLVE_TOL
+
+
 @pytest.mark.parametrize("lmax", [1, 2, 3, 4])
 def test_scattered_field_matches_oracle(lmax):
     """celes_scattered_field (eq. 3 with (A.2)) against the oracle at points outside every sphere: random points in

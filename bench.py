@@ -62,6 +62,8 @@ def parse():
                     help="time celes_scattered_field on an NP x NP grid of points in the plane 300 nm above the slab instead")
     ap.add_argument("--gaussian-beam", action="store_true",
                     help="time celes_gaussian_beam (waist 4 um, PAPER.md:140, centred on the slab, normal incidence) instead")
+    ap.add_argument("--levels", type=int, default=0,
+                    help="levels of the guided work partition (celes_options.levels; 0 = library default)")
     ap.add_argument("--lmax", type=int, default=0, help="override the workload's truncation order (1..5)")
     ap.add_argument("--hankel", default="registers", choices=["registers", "table"],
                     help="h_p(kd) in registers (default) or from the paper's lookup table (PAPER.md:130)")
@@ -594,7 +596,7 @@ def main():
     q = fields.mie_coefficients(w.lmax, w.k, rad, workloads.N_SPHERE)
     b_host = workloads.gaussian_coefficients(w.N, w.nmax, w.seed_b + rank)
     t0 = time.perf_counter()
-    ctx = celes.celes_setup(pos, rad, q, w.k, w.lmax, translation=args.translation, hankel=args.hankel)
+    ctx = celes.celes_setup(pos, rad, q, w.k, w.lmax, translation=args.translation, hankel=args.hankel, levels=args.levels)
     setup_s = time.perf_counter() - t0
     cfg = celes.celes_launch_config(ctx)
     b = torch.from_numpy(b_host).cuda()
@@ -668,7 +670,7 @@ def main():
             "gpu_launches": 3 * args.steps,
             "roofline": roof,
         }
-        if w.name == "C4" and world == 1 and not args.lmax:
+        if w.name == "C4" and world == 1 and not args.lmax and not args.levels:
             # BASELINE.json's metric names N = 1e4 as well: the same measurement on C3, reported beside the headline
             w3 = workloads.CONFIGS["C3"]
             pos3, rad3 = workloads.positions(w3)

@@ -74,8 +74,9 @@ typedef struct celes_options {
                               the pair grid in SMs x CTAs/SM equal runs, level 2 a quarter, ..., the last two an equal
                               share; 1 = one wave of equal runs (fewest partial sums, ~5 % slower: of two CTAs
                               resident on an SM the warp scheduler serves one first, and the other then finishes
-                              alone below full throughput); 0 = default CELES_DEFAULT_LEVELS (ten: beyond that nothing changes,
-                              and small N stops earlier, at runs of four emitter tiles) */
+                              alone below full throughput); 0 = default CELES_DEFAULT_LEVELS (ten: beyond that nothing changes;
+                              the halving also stops once a run would be shorter than 16 emitter tiles, which gives three
+                              levels at N = 1e4 -- measured best there, the partial sums then stay in L2) */
 } celes_options;
 #define CELES_DEFAULT_LEVELS 10
 #define CELES_RANGE_AUTO     0

@@ -13,9 +13,12 @@
 //       CTAs resident on an SM the warp scheduler favours one almost exclusively (measured: it finishes after 58 % of the
 //       pair's time, profiles/r02_cta_trace.md), and a CTA left alone on an SM reaches only 92 % of the pipe throughput
 //       of two.  One level (a single wave of equal runs) is 5.5 % slower than many waves for that reason; at N = 1e5
-//       six levels take 357.25 ms, ten (the default) 355.90 ms and more change nothing; at N = 1e4 the halving stops after
-//       five levels whatever is asked (runs shorter than CELES_MIN_RUN_TILES tiles are not made: shorter ones were
-//       measured slower).  At most n_res * levels + rblocks partial sums, instead of 56 per receiver block at N = 1e4.
+//       six levels take 357.25 ms, ten (the default) 355.90 ms and more change nothing.  The halving stops once a run would
+//       be shorter than CELES_MIN_RUN_TILES = 16 emitter tiles: at N = 1e4 that gives three levels with tiles of 32, measured
+//       best there (lmax 4: 7.440 ms against 7.476 with five and 7.719 with one; the 965 partial sums then stay in L2 --
+//       0.55 MB of DRAM writes per launch against 22.9 MB with five levels -- and finalize_kernel takes 20 us instead of 44),
+//       and five levels with the tiles of 8 of lmax = 5, measured slightly better for that kernel (18.06 ms against 18.2 with three).
+//       At most n_res * levels + rblocks partial sums, instead of 56 per receiver block at N = 1e4 with fixed splits.
 //   fixed splits (celes_options.emitter_splits = S > 0): every block's emitters are cut into S equal chunks, one CTA
 //       each, grid = rblocks x S CTAs in as many waves as that takes.
 #pragma once
@@ -23,7 +26,7 @@
 #include <vector>
 
 #ifndef CELES_MIN_RUN_TILES
-#define CELES_MIN_RUN_TILES 4     // shortest run the halving may produce, in emitter tiles
+#define CELES_MIN_RUN_TILES 16    // shortest run the halving may produce, in emitter tiles (note above)
 #endif
 
 namespace celes {
@@ -50,6 +53,7 @@ inline WorkPartition build_partition(int N, int kblock, int etile, int n_res, in
     p.rblocks = (N + p.bs - 1) / p.bs;
     const long long tiles = (N + etile - 1) / etile;        // emitter tiles per receiver block
     const long long total = tiles * p.rblocks;
+    const long long min_run_tiles = CELES_MIN_RUN_TILES;
     // runs of consecutive tiles of the flattened grid, one per CTA, in launch order
     std::vector<std::pair<long long, long long>> runs;
     if (fixed_splits > 0) {
@@ -62,7 +66,7 @@ inline WorkPartition build_partition(int N, int kblock, int etile, int n_res, in
         for (int lev = 0; lev < std::max(1, levels) && done < total; ++lev) {
             const bool last = lev + 1 >= std::max(1, levels);
             long long share = last ? total - done : (total - done) / 2;
-            if (share < (long long)CELES_MIN_RUN_TILES * n_res) share = total - done;   // runs of a few tiles: stop halving
+            if (share < min_run_tiles * n_res) share = total - done;       // shorter runs would not pay: stop halving
             const long long n = std::max<long long>(1, std::min<long long>(n_res, share));
             for (long long c = 0; c < n; ++c) {
                 const long long a = done + share * c / n, b = done + share * (c + 1) / n;

@@ -528,19 +528,28 @@ def solve_c5(celes, fields, workloads, translation, precond_edge=0.0):
     pc = None
     if precond_edge > 0:
         celes.celes_precond_setup(ctx, edge)                                      # warm-up
-    x.zero_()
-    torch.cuda.synchronize()
-    t0 = time.perf_counter()
-    if precond_edge > 0:
-        pc = celes.celes_precond_setup(ctx, edge)
+    # three complete runs (set-up + solve each); the MEDIAN is reported and every run is listed.  The solve is
+    # deterministic (same iterations every time) and repeats to 1 ms in isolation, but inside this script's full flow
+    # about one preconditioned run in three has come out 15-70 ms slow for a reason not found
+    runs = []
+    for _ in range(3):
+        x.zero_()
         torch.cuda.synchronize()
-    t_setup = time.perf_counter() - t0
-    info = celes.celes_solve(ctx, a_in, x, restart=30, rtol=1e-4, max_iters=2000, precond=pc is not None)
-    torch.cuda.synchronize()
-    sec = time.perf_counter() - t0
+        t0 = time.perf_counter()
+        if precond_edge > 0:
+            pc = celes.celes_precond_setup(ctx, edge)
+            torch.cuda.synchronize()
+        t_set = time.perf_counter() - t0
+        info = celes.celes_solve(ctx, a_in, x, restart=30, rtol=1e-4, max_iters=2000, precond=pc is not None)
+        torch.cuda.synchronize()
+        runs.append((time.perf_counter() - t0, t_set, info))
+    runs.sort(key=lambda r: r[0])
+    sec, t_setup, info = runs[1]
     out = {"workload": f"C5: N={w.N} lmax={w.lmax} plane wave +z x-pol, GMRES(30), rtol 1e-4", "seconds": sec,
+           "seconds_kind": "median of 3 complete runs (wall clock, set-up included)",
+           "seconds_all": [r[0] for r in runs], "library_solve_seconds_all": [r[2]["seconds"] for r in runs],
            "iterations": info["iterations"], "matvecs": info["matvecs"], "rel_residual": info["rel_residual"],
-           "converged": bool(info["converged"])}
+           "converged": bool(all(r[2]["converged"] for r in runs))}
     if pc is not None:
         out["preconditioner"] = dict(pc, edge_nm=precond_edge, setup_seconds=t_setup,
                                      setup_note="replaces a warm-up set-up on the same context: device memory is reused, no "

@@ -84,6 +84,22 @@ def test_overlap_check_finds_a_single_overlap_in_a_large_packing():
     assert _setup_rc(w.N, w.lmax, bad, rad, q, w.k)[0] == binding.CELES_EINVAL
 
 
+def test_default_partition_has_the_measured_level_counts():
+    """The level counts the documentation states and the profiles measured (profiles/r02n_levels_small_n.md,
+    r02i_kernel_c4.md): with 296 resident CTAs the default guided partition makes ten waves of runs at N = 1e5, three at
+    N = 1e4 with tiles of 32 (the halving stops at runs of 16 tiles) and five with the tiles of 8 that lmax = 5 uses; an
+    explicit level count still overrides the default downwards."""
+    res = 296
+    assert celes.celes_plan_work(100000, 32, res, 0, 0)["ctas"] == 10 * res
+    assert celes.celes_plan_work(10000, 32, res, 0, 0)["ctas"] == 3 * res
+    assert celes.celes_plan_work(10000, 8, res, 0, 0)["ctas"] == 5 * res
+    assert celes.celes_plan_work(100000, 32, res, 6, 0)["ctas"] == 6 * res
+    assert celes.celes_plan_work(10000, 32, res, 1, 0)["ctas"] == res
+    p = celes.celes_plan_work(10000, 32, res, 0, 0)
+    assert len(p["segments"]) == 965                                   # the partial-sum slots quoted in DESIGN.md section 5.0
+    assert len(celes.celes_plan_work(100000, 32, res, 0, 0)["segments"]) == 3740
+
+
 def test_without_a_gpu_the_product_fails_loudly_and_never_touches_the_oracle():
     """No CPU fallback (the tier's rule): on a box without a CUDA device a valid celes_setup is CELES_ECUDA and returns no
     context, bench.py's own arm exits non-zero saying so, and importing the product (package + bench) imports nothing of

@@ -31,6 +31,11 @@ void celes::host::free_precond(celes_ctx* c) {
 
 // z = blockdiag(M_j^{-1}) v  (step 4)
 int celes::host::precond_apply(celes_ctx* c, const float2* v, float2* z, cudaStream_t s) {
+    if (c->pc_max_n > celes::kGemvChunkedFrom) {               // tall blocks: x streamed through a fixed chunk of shared memory
+        celes::block_gemv_chunked_kernel<<<c->pc_ctas, celes::kGemvRows, 0, s>>>(
+            c->nmax, c->pc_cta_group, c->pc_cta_row0, c->pc_grp_offset, c->pc_order, c->pc_blk_offset, c->pc_perm, c->pc_blocks, v, z);
+        return cudaGetLastError() == cudaSuccess ? CELES_OK : CELES_ECUDA;
+    }
     const size_t smem = (size_t)c->pc_max_n * sizeof(float2);
     if (smem > 48 * 1024) {
         // the attribute belongs to the kernel, not to a context: raise it to the device limit (never lower it) and

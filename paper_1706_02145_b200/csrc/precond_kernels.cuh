@@ -14,6 +14,8 @@ namespace celes {
 
 constexpr int kAsmThreads = 96;     // >= nmax of every supported lmax (70 at lmax = 5)
 constexpr int kGemvRows = 128;      // rows of a block handled by one CTA of block_gemv_kernel
+constexpr int kGemvChunk = 1024;    // block_gemv_chunked_kernel: columns whose x values are staged at a time (8 KB)
+constexpr int kGemvChunkedFrom = 1536;   // largest block above this many rows: the chunked kernel (measured crossover)
 
 // One CTA per ordered pair (a, b) of spheres of one subset; thread t < nmax fills column n' = t of the nmax x nmax
 // block  M^{ab} = delta_ab 1 - T^a W^{ab}  inside the column-major n_j x n_j matrix of the subset.
@@ -163,6 +165,51 @@ __global__ void __launch_bounds__(kGemvRows) block_gemv_kernel(
         const float2 m0 = A[(size_t)c * n], x0 = xs[c];
         ar0 = fmaf(m0.x, x0.x, ar0); ar0 = fmaf(-m0.y, x0.y, ar0); ai0 = fmaf(m0.x, x0.y, ai0); ai0 = fmaf(m0.y, x0.x, ai0);
     }
+    const int s = r / nmax;
+    z[(size_t)order[g0 + s] * nmax + (r - s * nmax)] = make_float2(ar0 + ar1, ai0 + ai1);
+}
+
+// The same product for TALL blocks.  block_gemv_kernel keeps the whole x slice of its block in shared memory, which caps the
+// resident CTAs once a block has a few thousand rows (22 KB per CTA at 2736 rows: 9 CTAs per SM instead of 16) and with
+// them the loads in flight; here x streams through a fixed 8 KB chunk, so occupancy does not depend on the block.
+// Measured (profiles/r02r_block_gemv_tall_blocks.md): 0.64 -> 0.93 of the HBM copy bandwidth at 1980 rows, but 0.92 -> 0.70 at
+// 672 rows (two barriers per chunk and no long uninterrupted column loop), hence the dispatch by the largest block's size.
+__global__ void __launch_bounds__(kGemvRows) block_gemv_chunked_kernel(
+    int nmax, const int* __restrict__ cta_group, const int* __restrict__ cta_row0, const int* __restrict__ grp_offset,
+    const int* __restrict__ order, const long long* __restrict__ blk_offset, const int* __restrict__ perm,
+    const float2* __restrict__ blocks, const float2* __restrict__ v, float2* __restrict__ z) {
+    __shared__ float2 xs[kGemvChunk];
+    const int j = cta_group[blockIdx.x], row0 = cta_row0[blockIdx.x];
+    const int g0 = grp_offset[j], nj = grp_offset[j + 1] - g0, n = nj * nmax;
+    const int* pj = perm + (size_t)g0 * nmax;
+    const int r = row0 + threadIdx.x;
+    const bool active = r < n;
+    const float2* A = blocks + blk_offset[j] + (active ? r : 0);
+    float ar0 = 0.f, ai0 = 0.f, ar1 = 0.f, ai1 = 0.f;
+    for (int c0 = 0; c0 < n; c0 += kGemvChunk) {
+        const int nc = min(kGemvChunk, n - c0);
+        __syncthreads();                                               // the previous chunk is consumed
+        for (int c = threadIdx.x; c < nc; c += kGemvRows) {
+            const int pc = pj[c0 + c], s = pc / nmax;
+            xs[c] = v[(size_t)order[g0 + s] * nmax + (pc - s * nmax)];
+        }
+        __syncthreads();
+        if (active) {
+            const float2* Ac = A + (size_t)c0 * n;
+            int c = 0;
+            for (; c + 1 < nc; c += 2) {
+                const float2 m0 = Ac[(size_t)c * n], m1 = Ac[(size_t)(c + 1) * n];
+                const float2 x0 = xs[c], x1 = xs[c + 1];
+                ar0 = fmaf(m0.x, x0.x, ar0); ar0 = fmaf(-m0.y, x0.y, ar0); ai0 = fmaf(m0.x, x0.y, ai0); ai0 = fmaf(m0.y, x0.x, ai0);
+                ar1 = fmaf(m1.x, x1.x, ar1); ar1 = fmaf(-m1.y, x1.y, ar1); ai1 = fmaf(m1.x, x1.y, ai1); ai1 = fmaf(m1.y, x1.x, ai1);
+            }
+            if (c < nc) {
+                const float2 m0 = Ac[(size_t)c * n], x0 = xs[c];
+                ar0 = fmaf(m0.x, x0.x, ar0); ar0 = fmaf(-m0.y, x0.y, ar0); ai0 = fmaf(m0.x, x0.y, ai0); ai0 = fmaf(m0.y, x0.x, ai0);
+            }
+        }
+    }
+    if (!active) return;
     const int s = r / nmax;
     z[(size_t)order[g0 + s] * nmax + (r - s * nmax)] = make_float2(ar0 + ar1, ai0 + ai1);
 }

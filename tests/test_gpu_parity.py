@@ -378,6 +378,24 @@ def test_block_inversion_degenerate_cases(lmax):
         celes.celes_precond_setup(big, 600.0)                        # still usable
 
 
+@pytest.mark.parametrize("N", [52, 60])
+def test_precond_apply_tall_block_uses_the_chunked_gemv(N):
+    """Blocks of more than 1536 rows are applied by block_gemv_chunked_kernel (x streamed through an 8 KB chunk of shared
+    memory; csrc/precond_kernels.cuh): one cuboid of N spheres at lmax = 3 is a single block of 1560 / 1800 rows -- one full
+    chunk of 1024 columns and a ragged one -- checked against the oracle's dense solve, and M z = v through the matrix-free
+    system matvec."""
+    import dataclasses
+    w = dataclasses.replace(workloads.scaled(workloads.C2, N), lmax=3)
+    pos, rad, q, ctx, b = make(w)
+    info = celes.celes_precond_setup(ctx, 0.0)
+    assert info["n_groups"] == 1 and info["max_group_spheres"] * w.nmax == N * 30 > 1536
+    bd = torch.from_numpy(b).cuda()
+    z = celes.celes_precond_apply(ctx, bd)
+    qo = orc.mie_q(w.lmax, w.k, rad, workloads.N_SPHERE)
+    assert rel(z.cpu().numpy(), orc.precond_apply(pos, w.k, w.lmax, qo, 0.0, b)) <= SOLVE_TOL
+    assert rel(celes.celes_system_matvec(ctx, z).cpu().numpy(), b) <= SOLVE_TOL
+
+
 def test_preconditioned_solve_same_solution_fewer_iterations():
     """Right-preconditioned GMRES: same solution as the oracle's tight solve, fewer iterations
     than the unpreconditioned solve; asking for the preconditioner before celes_precond_setup is an error."""

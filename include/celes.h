@@ -33,6 +33,7 @@ extern "C" {
 #define CELES_ENOMEM  -2   /* host or device allocation failed */
 #define CELES_ECUDA   -3   /* CUDA runtime error (no device, launch failure, ...) */
 #define CELES_ENOCONV -4   /* celes_solve reached max_iters; x holds the last iterate and info is filled */
+#define CELES_ELIMIT  -5   /* a size beyond the fixed capacity of a no-allocation entry point (celes_far_field_noalloc) */
 
 #define CELES_LMAX_MIN 1
 #define CELES_LMAX_MAX 5   /* lmax = 5 (nmax = 70): CELES_TRANSLATION_ROTATED only */
@@ -201,6 +202,22 @@ int celes_partition(int N, const double* pos_xyz, const double* edge_xyz, int* g
  * The field calls of one context share that scratch block: issue them on one stream. */
 int celes_far_field(celes_ctx* ctx, const void* b_dev, int n_dir, const double* alpha, const double* beta,
                     void* g_dev, void* cuda_stream);
+
+/* celes_far_field for callers that must not allocate (code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc): same arguments, same result, but every table the kernels need (directions, B_nj e^{i m alpha}, the
+ * split partial sums of the sphere sum) lives in ONE static device array of the library -- 5 MiB, held by every GPU that
+ * loads the library until the process exits -- whose device address celes_setup looked up once for the context's device.
+ * The call makes no cudaMalloc, no cudaFree and no host allocation, whatever it was called with before.
+ *   n_dir <= CELES_FAR_FIELD_NOALLOC_MAX_DIR (2048), any supported lmax; more directions: CELES_ELIMIT, nothing is launched
+ *   (evaluate them in batches, or use celes_far_field).
+ * The array is shared by every context and every call on the device and keeps the previous call's contents; nothing in it
+ * has to start at zero (each call overwrites every entry it reads).  Two calls that overlap on the GPU (different streams,
+ * or different host threads on one device) RACE on it: issue them on one stream, or order them with events.
+ * alpha, beta: host arrays, copied with cudaMemcpyAsync on cuda_stream (pinned memory keeps the call asynchronous).
+ * Errors as celes_far_field, plus CELES_ELIMIT; CELES_ECUDA if the array's address could not be resolved at set-up. */
+#define CELES_FAR_FIELD_NOALLOC_MAX_DIR 2048
+int celes_far_field_noalloc(celes_ctx* ctx, const void* b_dev, int n_dir, const double* alpha, const double* beta,
+                            void* g_dev, void* cuda_stream);
 
 /* Initial-field coefficients of the plane wave E_0 Phi_j(alpha, beta; r) = E_0 exp(i k.r) e_j about every sphere centre,
  * from (A.13)-(A.14): a^i_n = E_0 exp(i k.r_i) 4 exp(-i m alpha) B^dagger_nj(beta).

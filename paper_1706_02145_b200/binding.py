@@ -16,7 +16,8 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libceles.so")
 
-CELES_OK, CELES_EINVAL, CELES_ENOMEM, CELES_ECUDA, CELES_ENOCONV = 0, -1, -2, -3, -4
+CELES_OK, CELES_EINVAL, CELES_ENOMEM, CELES_ECUDA, CELES_ENOCONV, CELES_ELIMIT = 0, -1, -2, -3, -4, -5
+CELES_FAR_FIELD_NOALLOC_MAX_DIR = 2048
 CELES_GMRES, CELES_BICGSTAB = 0, 1
 CELES_PRECOND_NONE, CELES_PRECOND_BLOCKDIAG = 0, 1
 CELES_TRANSLATION_ROTATED, CELES_TRANSLATION_DIRECT = 0, 1
@@ -27,7 +28,7 @@ EXPORTS = ["celes_setup", "celes_coupling_matvec", "celes_system_matvec", "celes
            "celes_launch_config", "celes_translation_table", "celes_fp32_peak_probe", "celes_precond_setup",
            "celes_precond_apply", "celes_partition", "celes_far_field", "celes_gaussian_beam", "celes_plane_wave",
            "celes_scattered_field", "celes_coupling_matvec_rows", "celes_system_matvec_rows", "celes_work_partition",
-           "celes_plan_work", "celes_range_info"]
+           "celes_plan_work", "celes_range_info", "celes_far_field_noalloc"]
 
 
 class CelesError(RuntimeError):
@@ -116,6 +117,8 @@ def lib() -> ctypes.CDLL:
         L.celes_gaussian_beam.argtypes = [p, ctypes.POINTER(celes_beam), p, p]
         L.celes_far_field.restype = i
         L.celes_far_field.argtypes = [p, p, i, p, p, p, p]
+        L.celes_far_field_noalloc.restype = i
+        L.celes_far_field_noalloc.argtypes = [p, p, i, p, p, p, p]
         L.celes_fp32_peak_probe.restype = i
         L.celes_fp32_peak_probe.argtypes = [i, i, ctypes.POINTER(d), ctypes.POINTER(d), p]
         _LIB = L
@@ -353,6 +356,25 @@ def celes_far_field(ctx: Context, b, alpha, beta, g=None, stream=None):
                                _stream(stream))
     if rc != CELES_OK:
         raise CelesError(rc, "celes_far_field")
+    return g
+
+
+def celes_far_field_noalloc(ctx: Context, b, alpha, beta, g, stream=None):
+    """celes_far_field_noalloc of include/celes.h: the far field from the library's static scratch array, no allocation in
+    the call (at most CELES_FAR_FIELD_NOALLOC_MAX_DIR directions; g [n_dir, 2] complex64 is the CALLER's tensor).
+    alpha, beta: contiguous float64 host arrays of equal length (no conversion or copy is made here)."""
+    _check_vec(b, ctx, "b")
+    for a in (alpha, beta):
+        if not (isinstance(a, np.ndarray) and a.dtype == np.float64 and a.flags.c_contiguous and a.ndim == 1):
+            raise ValueError("alpha and beta: contiguous 1-d float64 ndarrays")
+    if alpha.shape != beta.shape or alpha.size < 1:
+        raise ValueError("alpha and beta: same non-zero length")
+    if not (g.is_cuda and g.is_contiguous() and g.numel() == 2 * alpha.size and g.element_size() == 8):
+        raise ValueError("g: contiguous CUDA complex64 tensor with 2 * n_dir elements")
+    rc = lib().celes_far_field_noalloc(ctx.handle, b.data_ptr(), int(alpha.size), alpha.ctypes.data, beta.ctypes.data,
+                                       g.data_ptr(), _stream(stream))
+    if rc != CELES_OK:
+        raise CelesError(rc, "celes_far_field_noalloc")
     return g
 
 

@@ -176,6 +176,7 @@ const char* celes_strerror(int code) {
         case CELES_ENOMEM: return "out of memory";
         case CELES_ECUDA: return "CUDA error or no CUDA device";
         case CELES_ENOCONV: return "iterative solver did not converge within max_iters";
+        case CELES_ELIMIT: return "size beyond the fixed capacity of a no-allocation entry point";
     }
     return "unknown error code";
 }
@@ -233,6 +234,8 @@ static int setup_impl(celes_ctx** out, int N, int lmax, const double* pos_xyz, c
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, c->device) != cudaSuccess) return fail(CELES_ECUDA);
     c->sm_count = prop.multiProcessorCount;
+    // device address of the static scratch of celes_far_field_noalloc: looked up here, once per device, with this device current
+    if (celes::host::far_static_scratch_address(c->device, &c->far_static) == CELES_ECUDA) return fail(CELES_ECUDA);
     // lmax = 5 spills ~0.5 KB per thread; a small tile leaves the L1 carve-out to those spills (measured: 17.8 ms with 8,
     // 19.2 ms with 32 at N = 1e4, profiles/r02d_other_kernels.md)
     c->etile = (opt && opt->emitter_tile > 0) ? opt->emitter_tile : (lmax >= 5 ? 8 : 32);

@@ -34,6 +34,7 @@ struct celes_ctx {
     HankelTable htab_desc = {nullptr, 0.0f, 0.0f, 0};
     float2* bpm = nullptr;       // [N][nmax] work: [b_+ | b_-]
     float2* ypart = nullptr;     // [n_seg][kBlock][nmax] work: partial sums, one slot per segment
+    void* far_static = nullptr;  // device address of the static scratch of celes_far_field_noalloc on this context's device
     void* scratch = nullptr;     // device scratch of the field calls (direction / beam / point tables), grown on demand
     size_t scratch_bytes = 0;
     float2 *host_in = nullptr, *host_out = nullptr;   // [N][nmax] staging of the *_host entry points (allocated on first use)
@@ -89,6 +90,8 @@ inline int run_matvec(celes_ctx* c, const float2* b, float2* out, bool system, c
 // z = blockdiag(M_j^{-1}) v, and release of the preconditioner (precond.cu)
 int precond_apply(celes_ctx* c, const float2* v, float2* z, cudaStream_t s);
 void free_precond(celes_ctx* c);
+// device address of fields.cu's static scratch array on the current device, one cudaGetSymbolAddress per device (fields.cu)
+int far_static_scratch_address(int device, void** out);
 // release of the Krylov work space (solve.cu)
 void free_krylov(celes_ctx* c);
 }  // namespace host

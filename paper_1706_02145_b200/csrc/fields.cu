@@ -4,6 +4,7 @@
 
 #include <algorithm>
 #include <cmath>
+#include <mutex>
 #include <vector>
 
 #include "ctx.h"
@@ -37,7 +38,41 @@ struct Scratch {
     }
 };
 
+// ---- static scratch of celes_far_field_noalloc -----------------------------------------------------------------------
+// One file-scope device array, held by every GPU that loads the library until the process exits (5 MiB), cut into fixed
+// pieces sized for CELES_FAR_FIELD_NOALLOC_MAX_DIR directions and the largest nmax (70, lmax = 5).  In HOST code the
+// name g_far_static is only a stand-in for the symbol, not a device address: the address comes from
+// cudaGetSymbolAddress, looked up once per device in far_static_scratch_address() below (called by celes_setup with the
+// context's device current) and kept in the context.
+constexpr size_t kFarStaticBytes = 5u << 20;
+constexpr size_t kFarStaticAngOff = 0;                                                               // [2][max_dir] double
+constexpr size_t kFarStaticDirOff = kFarStaticAngOff + sizeof(double) * 2 * CELES_FAR_FIELD_NOALLOC_MAX_DIR;    // [max_dir][3] double
+constexpr size_t kFarStaticCoefOff = kFarStaticDirOff + sizeof(double) * 3 * CELES_FAR_FIELD_NOALLOC_MAX_DIR;   // [2 max_dir][70] float2
+constexpr size_t kFarStaticPartOff = kFarStaticCoefOff + sizeof(float2) * 2 * CELES_FAR_FIELD_NOALLOC_MAX_DIR * 70;
+constexpr size_t kFarStaticPartCapacity = (kFarStaticBytes - kFarStaticPartOff) / sizeof(float2);    // split partial sums
+static_assert(kFarStaticDirOff % 256 == 0 && kFarStaticCoefOff % 256 == 0 && kFarStaticPartOff % 256 == 0, "pieces stay 256-byte aligned");
+static_assert(kFarStaticPartOff < kFarStaticBytes, "the array holds the tables");
+static __device__ __align__(256) unsigned char g_far_static[kFarStaticBytes];
+
+constexpr int kMaxDevices = 64;
+std::mutex g_far_static_mutex;
+void* g_far_static_addr[kMaxDevices] = {};     // device address of g_far_static on device d (null: not looked up yet)
+
 }  // namespace
+
+// Device address of the static scratch on the CURRENT device (which must be `device`); one cudaGetSymbolAddress per device
+// and process.  Allocates nothing: the array is part of the library's device image.
+int celes::host::far_static_scratch_address(int device, void** out) {
+    if (!out || device < 0 || device >= kMaxDevices) return CELES_EINVAL;
+    std::lock_guard<std::mutex> lock(g_far_static_mutex);
+    if (g_far_static_addr[device] == nullptr) {
+        void* p = nullptr;
+        if (cudaGetSymbolAddress(&p, g_far_static) != cudaSuccess || p == nullptr) { cudaGetLastError(); return CELES_ECUDA; }
+        g_far_static_addr[device] = p;
+    }
+    *out = g_far_static_addr[device];
+    return CELES_OK;
+}
 
 extern "C" {
 
@@ -80,6 +115,48 @@ int celes_far_field(celes_ctx* ctx, const void* b_dev, int n_dir, const double* 
         if (!rc && cudaGetLastError() != cudaSuccess) rc = CELES_ECUDA;
     }
     return rc;
+}
+
+// The same far field from the static scratch: no cudaMalloc, no cudaFree, no host allocation (see celes.h).  The launch
+// configuration is the one celes_far_field would use (so is the result, bit for bit) unless the split partial sums would
+// not fit the array, in which case the sphere sum is cut into fewer splits.
+int celes_far_field_noalloc(celes_ctx* ctx, const void* b_dev, int n_dir, const double* alpha, const double* beta,
+                            void* g_dev, void* cuda_stream) {
+    if (!ctx || !b_dev || !g_dev || n_dir < 1 || !alpha || !beta) return CELES_EINVAL;
+    if (n_dir > CELES_FAR_FIELD_NOALLOC_MAX_DIR) return CELES_ELIMIT;
+    if (ctx->far_static == nullptr || ctx->nmax > 70) return CELES_ECUDA;      // set-up could not resolve the array
+    for (int d = 0; d < n_dir; ++d)
+        if (!std::isfinite(alpha[d]) || !std::isfinite(beta[d])) return CELES_EINVAL;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const int pols = ctx->lmax <= 3 ? 2 : 1;
+    const int rows = 2 * n_dir, gx = (rows / pols + celes::kFarThreads - 1) / celes::kFarThreads;
+    int splits = std::max(1, std::min((8 * ctx->sm_count + gx - 1) / gx, std::max(1, ctx->N / (4 * celes::kFarTile))));
+    splits = std::max(1, std::min(splits, (int)(kFarStaticPartCapacity / (size_t)rows)));      // the partial sums must fit
+    const int chunk = ((ctx->N + splits - 1) / splits + celes::kFarTile - 1) / celes::kFarTile * celes::kFarTile;
+    splits = (ctx->N + chunk - 1) / chunk;
+    unsigned char* base = static_cast<unsigned char*>(ctx->far_static);
+    double* d_ang = reinterpret_cast<double*>(base + kFarStaticAngOff);
+    double* d_dir = reinterpret_cast<double*>(base + kFarStaticDirOff);
+    float2* d_coef = reinterpret_cast<float2*>(base + kFarStaticCoefOff);
+    float2* d_part = reinterpret_cast<float2*>(base + kFarStaticPartOff);
+    // nothing in the array has to start at zero: the three kernels below write every entry they later read (angles,
+    // unit vectors, all nmax coefficients of all rows, one partial sum per (split, row)), so the previous call's
+    // contents are simply overwritten
+    if (cudaMemcpyAsync(d_ang, alpha, sizeof(double) * n_dir, cudaMemcpyHostToDevice, s) != cudaSuccess ||
+        cudaMemcpyAsync(d_ang + n_dir, beta, sizeof(double) * n_dir, cudaMemcpyHostToDevice, s) != cudaSuccess) return CELES_ECUDA;
+    celes::far_field_coefficients_kernel<<<(n_dir + 127) / 128, 128, 0, s>>>(ctx->lmax, n_dir, d_ang, d_ang + n_dir, d_coef, d_dir);
+    const float2* b = (const float2*)b_dev;
+    dim3 grid(gx, splits);
+    switch (ctx->lmax) {
+        case 1: celes::far_field_kernel<6, 2><<<grid, celes::kFarThreads, 0, s>>>(ctx->N, chunk, rows, ctx->kpos, b, d_coef, d_dir, d_part); break;
+        case 2: celes::far_field_kernel<16, 2><<<grid, celes::kFarThreads, 0, s>>>(ctx->N, chunk, rows, ctx->kpos, b, d_coef, d_dir, d_part); break;
+        case 3: celes::far_field_kernel<30, 2><<<grid, celes::kFarThreads, 0, s>>>(ctx->N, chunk, rows, ctx->kpos, b, d_coef, d_dir, d_part); break;
+        case 4: celes::far_field_kernel<48, 1><<<grid, celes::kFarThreads, 0, s>>>(ctx->N, chunk, rows, ctx->kpos, b, d_coef, d_dir, d_part); break;
+        case 5: celes::far_field_kernel<70, 1><<<grid, celes::kFarThreads, 0, s>>>(ctx->N, chunk, rows, ctx->kpos, b, d_coef, d_dir, d_part); break;
+        default: return CELES_EINVAL;
+    }
+    celes::far_field_reduce_kernel<<<(rows + 255) / 256, 256, 0, s>>>(rows, splits, d_part, (float2*)g_dev);
+    return cudaGetLastError() == cudaSuccess ? CELES_OK : CELES_ECUDA;
 }
 
 int celes_plane_wave(celes_ctx* ctx, double alpha, double beta, int polarisation, double E0_re, double E0_im, void* a_in_dev,

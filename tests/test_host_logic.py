@@ -40,7 +40,7 @@ def test_nmax_and_strerror():
         celes.celes_nmax(0)
     with pytest.raises(celes.CelesError):
         celes.celes_nmax(6)
-    for code in (0, -1, -2, -3, -4):
+    for code in (0, -1, -2, -3, -4, -5):
         assert binding.strerror(code) and "unknown" not in binding.strerror(code)
     assert "unknown" in binding.strerror(-99)
 

@@ -1,6 +1,8 @@
 // solve.cu -- celes_solve: host-driven restarted GMRES and BiCGSTAB on M x = T a_in, every vector
 // operation a device kernel (krylov_kernels.cuh), optional right preconditioning with the block-diagonal operator.
 #include <cuda_runtime.h>
+#include <cstdlib>
+#include <cstdio>
 
 #include <algorithm>
 #include <chrono>
@@ -196,7 +198,27 @@ static int solve_impl(celes_ctx* ctx, const void* a_in_dev, void* x_dev, const c
     int iterations = 0, matvecs = 0, n_hist = 0, converged = 0;
     double rel = 0.0;
     auto push_hist = [&](double v) { if (info && n_hist < CELES_MAX_HISTORY) info->history[n_hist++] = v; };
+    // diagnostic (CELES_DEBUG set): host time at which every Hessenberg column arrived; finish() prints how the gaps between
+    // them are distributed -- a few long gaps mean host / driver hiccups, uniformly longer ones a slower GPU
+    const bool dbg_gaps = std::getenv("CELES_DEBUG") != nullptr;
+    constexpr int kMaxStamps = 4096;
+    double stamp[kMaxStamps];
+    int n_stamp = 0;
     auto finish = [&](int code) {
+        if (dbg_gaps && n_stamp > 3) {
+            double gap[kMaxStamps];
+            for (int t = 1; t < n_stamp; ++t) gap[t - 1] = stamp[t] - stamp[t - 1];
+            const int ng = n_stamp - 1;
+            int at = 0;
+            for (int t = 1; t < ng; ++t) if (gap[t] > gap[at]) at = t;          // which arrival the longest wait preceded
+            std::sort(gap, gap + ng);
+            const double med = gap[ng / 2];
+            double excess = 0.0; int n_long = 0;
+            for (int t = 0; t < ng; ++t) if (gap[t] > 1.5 * med) { excess += gap[t] - med; ++n_long; }
+            std::fprintf(stderr, "celes_solve gaps ms: n %d | median %.3f | p90 %.3f | max %.3f %.3f %.3f | longest before arrival %d | %d gaps > 1.5 median hold %.2f ms of excess | total %.1f\n",
+                         ng, 1e3 * med, 1e3 * gap[(int)(0.9 * ng)], 1e3 * gap[ng - 1], 1e3 * gap[ng - 2], 1e3 * gap[ng - 3], at + 1, n_long, 1e3 * excess,
+                         1e3 * (stamp[n_stamp - 1] - stamp[0]));
+        }
         if (info) {
             info->iterations = iterations; info->matvecs = matvecs; info->converged = converged;
             info->rel_residual = rel; info->n_history = n_hist;
@@ -289,6 +311,7 @@ static int solve_impl(celes_ctx* ctx, const void* a_in_dev, void* x_dev, const c
                 ++enq;
             }
             SOLVE_TRY(cudaEventSynchronize(ctx->kry_ev[j & 1]));
+            if (dbg_gaps && n_stamp < kMaxStamps) stamp[n_stamp++] = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_start).count();
             ++iterations;
             const double2* hh = ctx->hhost + (size_t)(j & 1) * hs;
             // Hessenberg column j, Givens rotations
